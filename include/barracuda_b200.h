@@ -1,0 +1,156 @@
+/* barracuda_b200.h -- C-ABI boundary of the B200-native inexact backward search.
+ *
+ * What the library computes: for every read of a batch and for both strands, the set of
+ * suffix-array intervals [k,l] of every reference substring that aligns to the query within the
+ * difference budgets (mismatches + gap opens + gap extensions <= z, a 5' seed with its own limit),
+ * deduplicated, sorted, with the minimum difference count per interval.
+ *
+ * Where the paper defines the operations (PAPER.md = /root/reference/PAPER.md, a prose-only note):
+ *   - index wholly resident in GPU memory:                 PAPER.md:64 (sec. 2), :41, :86 (sec. 3.4)
+ *   - two pointers k,l updated per base from the index, l-k+1 = number of matches,
+ *     crossing = absent:                                   PAPER.md:62 (sec. 2)
+ *   - "carefully back up its search and start trying out alternatives" (inexact search):
+ *                                                          PAPER.md:62
+ *   - hundreds of thousands of reads per launch:
+ *   - "zero or more possible alignments" per read:         PAPER.md:100 (sec. 3.7)
+ *   - coordinates are needed by the next step (sampe):
+ * Everything the paper leaves open (difference model, gap rules, seed, strands, $ handling,
+ * limits) is fixed in DESIGN.md "Readings of the paper" (= SURVEY.md 8c, C1..C7).
+ *
+ * Conventions
+ *   - Every function returns BC_OK (0) or a negative bc_status; nothing throws, aborts or prints.
+ *   - The library allocates NO device memory: the caller (PyTorch in this repo) owns every device
+ *     buffer; sizes come from the *_bytes calls.  "host" / "device" is stated per pointer.
+ *   - Host inputs are borrowed for the duration of the call only.
+ *   - All work is enqueued on the given CUDA stream (a cudaStream_t passed as void*, NULL = legacy
+ *     default stream).  bc_index_upload, bc_align_batch and bc_locate synchronise that stream
+ *     before returning, so status codes are final.
+ *   - Deterministic: same inputs -> byte-identical outputs whatever the scheduling.
+ *   - One bc_index may be used from one host thread at a time.  No CPU fallback exists.
+ *   - Alphabet A,C,G,T = 0..3; N (reads only) is flagged in a separate mask; complement = 3-c.
+ */
+#ifndef BARRACUDA_B200_H
+#define BARRACUDA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BC_OK = 0,
+    BC_E_INVAL = -1,       /* bad argument (NULL, len 0 or > 256, z > 255, negative option, n >= 2^32-1, ...) */
+    BC_E_NOMEM = -2,       /* a caller-provided buffer (d_mem, workspace) is smaller than *_bytes said */
+    BC_E_CUDA = -3,        /* a CUDA runtime call or kernel failed */
+    BC_E_OVERFLOW = -4,    /* raw-hit arena or hits_capacity too small; see bc_result.n_hits_needed */
+    BC_E_UNSUPPORTED = -5
+} bc_status;
+
+#define BC_MAX_READ_LEN 256
+
+/* One BWT.  X = T$, '$' smallest; SA = suffix array of X (n+1 rows, SA[0] = n);
+ * B[j] = X[SA[j]-1]; B[primary] = '$'.  HOST memory. */
+typedef struct {
+    uint64_t n;               /* |T|, 1 <= n < 2^32-1 */
+    uint64_t primary;         /* row whose BWT symbol is '$' (SA[primary] = 0) */
+    const uint64_t *bwt2;     /* n symbols, '$' removed, 2 bits each: symbol j at bits 2*(j%32) of word j/32 */
+    uint32_t occ_interval;    /* multiple of 32 */
+    const uint32_t *occ;      /* [n/occ_interval + 1][4]: occurrences of A,C,G,T before symbol t*occ_interval */
+    uint64_t C[5];            /* C[c] = #{t : T[t] < c}; C[4] = n */
+} bc_bwt_host;
+
+/* fwd = BWT of T; rev = BWT of reverse(T) (not complemented); sa[t] = SA_fwd[t*sa_interval],
+ * t = 0 .. n/sa_interval (rows of the full n+1-row suffix array).  HOST memory. */
+typedef struct {
+    bc_bwt_host fwd, rev;
+    uint32_t sa_interval;     /* >= 1 */
+    const uint32_t *sa;
+} bc_index_host;
+
+/* Search options: d = mismatches + gap opens + gap extensions <= z; totals
+ * n_go <= max_gap_open, n_ge <= max_gap_ext; seed = first seed_len bases of the read (5' end),
+ * enabled iff 0 < seed_len < len, differences inside it <= seed_z; a gap column needs
+ * >= indel_end_skip read bases on either side. */
+typedef struct {
+    int32_t z, max_gap_open, max_gap_ext, seed_len, seed_z, indel_end_skip;
+} bc_opts;
+
+/* A batch of reads.  DEVICE memory, borrowed. */
+typedef struct {
+    const uint32_t *bases2;   /* base i of the stream at bits 2*(i%16) of word i/16 (N stored as 0) */
+    const uint32_t *nmask;    /* bit i%32 of word i/32 set iff base i is N; NULL = no N anywhere */
+    const uint64_t *off;      /* [n_reads] first base of read r in the stream */
+    const uint16_t *len;      /* [n_reads] 1..BC_MAX_READ_LEN */
+    uint32_t n_reads;
+} bc_reads;
+
+typedef struct { uint32_t k, l; uint8_t d, strand; uint16_t zero; } bc_hit;   /* 12 bytes */
+
+/* Output, DEVICE memory, caller-owned.  For read r the hits are hits[hit_offsets[r] ..
+ * hit_offsets[r+1]): strand 0 (query = read) first, then strand 1 (query = revcomp(read)), each
+ * sorted by (k,l); [k,l] are rows of the FORWARD suffix array for both strands. */
+typedef struct {
+    uint64_t *hit_offsets;    /* [n_reads+1] */
+    bc_hit *hits;
+    uint64_t hits_capacity;   /* in hits */
+    uint64_t *n_hits_needed;  /* [2]: [0] = total hits after dedup, [1] = raw (pre-dedup) records the
+                                 search produced.  Both valid on BC_E_OVERFLOW unless the raw arena
+                                 itself overflowed, in which case only [1] is (grow the workspace). */
+} bc_result;
+
+typedef struct bc_index bc_index;   /* opaque handle (host object holding device pointers) */
+
+/* Bytes of device memory bc_index_upload needs for this index (lines of both BWTs, SA sample,
+ * staging for the transport arrays). */
+int bc_index_device_bytes(const bc_index_host *h, size_t *bytes);
+
+/* Copies the transport arrays to the device and re-lays them out (kernel) into 64-byte lines:
+ * {uint32 cnt[4]; uint64 lo[3]; uint64 hi[3]} = occurrences of A,C,G,T before symbol 192*i and
+ * the two bit-planes of symbols 192*i .. 192*i+191, so that one rank query O(.,j) for all four
+ * symbols reads exactly one line (north_star).  d_mem: DEVICE, 256-byte aligned,
+ * >= bc_index_device_bytes, owned by the caller and must outlive the handle. */
+int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_bytes, void *cuda_stream, bc_index **out);
+
+/* Frees the handle only; d_mem stays the caller's. */
+int bc_index_free(bc_index *ix);
+
+/* Workspace bytes for a batch: fixed part (prepared queries with their D[] bounds, per-warp state
+ * pools, counters) + a raw-hit arena of raw_hits_per_read * n_reads records (0 = default 16). */
+int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t max_len, const bc_opts *o,
+                             uint32_t raw_hits_per_read, size_t *bytes);
+
+/* The hot path: D[] bounds, inexact search of both strands 5'->3', hit emission,
+ * per-read sort + dedup -> CSR.  d_workspace: DEVICE, 256-byte aligned; whatever ws_bytes exceeds
+ * the fixed part becomes the raw-hit arena.  Returns BC_E_OVERFLOW (never truncates) when the arena
+ * or hits_capacity is too small; the output is then undefined except n_hits_needed. */
+int bc_align_batch(const bc_index *ix, const bc_reads *reads, const bc_opts *o, bc_result *res,
+                   void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
+/* SA-interval row -> text coordinate: pos[i] = SA_fwd[rows[i]] by LF-walk to
+ * a sampled row.  d_rows, d_pos: DEVICE.  rows[i] must be in [0, n]. */
+int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream);
+
+/* Device-side counters of the last bc_align_batch on this index (HOST out array of 8 uint64):
+ * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] 64-byte lines fetched,
+ * [3] raw hits, [4] D-kernel lookups, [5] pool high-water mark, [6] search-kernel ns (0 if not
+ * timed), [7] reserved. */
+int bc_last_stats(const bc_index *ix, uint64_t *out8);
+
+/* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM, warps per CTA. */
+int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
+
+/* Host-side index construction for synthetic genomes (untimed helper): suffix sort
+ * of T$ and reverse(T)$ -> transport arrays.  text: HOST, n codes 0..3.  The arrays are allocated
+ * by the library and released with bc_index_host_free. */
+int bc_index_build_host(const uint8_t *text, uint64_t n, uint32_t occ_interval, uint32_t sa_interval,
+                        int n_threads, bc_index_host **out);
+int bc_index_host_free(bc_index_host *h);
+
+const char *bc_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BARRACUDA_B200_H */

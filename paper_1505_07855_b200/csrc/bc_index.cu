@@ -1,0 +1,196 @@
+// bc_index_upload (A0 re-layout kernel), bc_locate (A7), handle management.  sm_100a only.
+#include <new>
+
+#include "bc_internal.cuh"
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t lines_bytes, off_fwd, off_rev, off_sa, sa_bytes, off_stage_bwt, stage_bwt_bytes, off_stage_occ,
+        stage_occ_bytes, total;
+    uint64_t n_lines;
+};
+
+bool check_bwt(const bc_bwt_host &b) {
+    return b.bwt2 && b.occ && b.n >= 1 && b.n < 0xFFFFFFFFull && b.primary <= b.n && b.occ_interval > 0 &&
+           b.occ_interval % 32 == 0 && b.C[4] == b.n;
+}
+
+int make_layout(const bc_index_host *h, Layout &L) {
+    if (!h || !h->sa || h->sa_interval == 0 || !check_bwt(h->fwd) || !check_bwt(h->rev) || h->fwd.n != h->rev.n)
+        return BC_E_INVAL;
+    uint64_t n = h->fwd.n;
+    L.n_lines = n / BC_LINE_SYMS + 1;
+    L.lines_bytes = align_up(L.n_lines * 64, 256);
+    L.off_fwd = 0;
+    L.off_rev = L.lines_bytes;
+    L.off_sa = 2 * L.lines_bytes;
+    L.sa_bytes = align_up((n / h->sa_interval + 1) * 4, 256);
+    L.off_stage_bwt = L.off_sa + L.sa_bytes;
+    L.stage_bwt_bytes = align_up((n / 32 + 1) * 8, 256);
+    L.off_stage_occ = L.off_stage_bwt + L.stage_bwt_bytes;
+    uint32_t oi = h->fwd.occ_interval < h->rev.occ_interval ? h->fwd.occ_interval : h->rev.occ_interval;
+    L.stage_occ_bytes = align_up((n / oi + 1) * 16, 256);
+    L.total = L.off_stage_occ + L.stage_occ_bytes;
+    return BC_OK;
+}
+
+// even bits of x (bit 2i -> bit i)
+__device__ __forceinline__ uint32_t compact_even(uint64_t x) {
+    x &= 0x5555555555555555ull;
+    x = (x | (x >> 1)) & 0x3333333333333333ull;
+    x = (x | (x >> 2)) & 0x0F0F0F0F0F0F0F0Full;
+    x = (x | (x >> 4)) & 0x00FF00FF00FF00FFull;
+    x = (x | (x >> 8)) & 0x0000FFFF0000FFFFull;
+    x = (x | (x >> 16)) & 0x00000000FFFFFFFFull;
+    return (uint32_t)x;
+}
+
+// A0: one thread per 64-byte line
+__global__ void bc_relayout_kernel(const uint64_t *__restrict__ bwt2, const uint32_t *__restrict__ occ,
+                                   uint32_t occ_interval, uint64_t n, uint64_t n_lines, BcLine *__restrict__ out) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_lines) return;
+    uint64_t s0 = i * BC_LINE_SYMS;                  // first symbol of the line (may be == n: empty tail line)
+    uint64_t n_words = n / 32 + 1;
+    uint64_t t = s0 / occ_interval;
+    uint32_t cnt[4];
+    for (int c = 0; c < 4; ++c) cnt[c] = occ[t * 4 + c];
+    for (uint64_t w = t * occ_interval / 32; w < s0 / 32; ++w) {   // whole words between checkpoint and line start
+        uint64_t x = bwt2[w], lo = x & 0x5555555555555555ull, hi = (x >> 1) & 0x5555555555555555ull;
+        uint32_t nt = __popcll(lo & hi), nc = __popcll(lo & ~hi), ng = __popcll(hi & ~lo);
+        cnt[0] += 32 - nt - nc - ng; cnt[1] += nc; cnt[2] += ng; cnt[3] += nt;
+    }
+    BcLine L;
+    for (int c = 0; c < 4; ++c) L.cnt[c] = cnt[c];
+    for (int q = 0; q < 3; ++q) {
+        uint64_t w0 = s0 / 32 + 2 * q;
+        uint64_t x0 = w0 < n_words ? bwt2[w0] : 0, x1 = w0 + 1 < n_words ? bwt2[w0 + 1] : 0;
+        L.lo[q] = (uint64_t)compact_even(x0) | ((uint64_t)compact_even(x1) << 32);
+        L.hi[q] = (uint64_t)compact_even(x0 >> 1) | ((uint64_t)compact_even(x1 >> 1) << 32);
+    }
+    out[i] = L;
+}
+
+// A7: one thread per row, LF-walk to a sampled row (one line per step)
+__global__ void bc_locate_kernel(BcIndexDev ix, const uint32_t *__restrict__ rows, uint64_t n_rows,
+                                 uint32_t *__restrict__ pos) {
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_rows) return;
+    const BcBwtDev &b = ix.bwt[0];
+    uint32_t j = rows[i], steps = 0;
+    if (j > b.n) { pos[i] = 0xFFFFFFFFu; return; }
+    while (j % ix.sa_interval != 0 && j != b.primary) {
+        uint32_t p = j - (j > b.primary ? 1u : 0u);           // index of B[j] in the '$'-less string
+        BcLineRegs L = bc_load_line(b.lines, p / BC_LINE_SYMS);
+        uint32_t r = p % BC_LINE_SYMS, c = bc_line_symbol(L, r), o[4];
+        bc_line_rank4(L, r, o);
+        j = b.C[c] + o[c] + 1;                                // C[c] + O(c, j), O counts B[0..j] inclusive
+        ++steps;
+    }
+    pos[i] = (j == b.primary ? 0u : ix.sa[j / ix.sa_interval]) + steps;
+}
+
+}  // namespace
+
+extern "C" int bc_index_device_bytes(const bc_index_host *h, size_t *bytes) {
+    Layout L;
+    if (!bytes) return BC_E_INVAL;
+    int rc = make_layout(h, L);
+    if (rc) return rc;
+    *bytes = L.total;
+    return BC_OK;
+}
+
+extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_bytes, void *cuda_stream, bc_index **out) {
+    Layout L;
+    if (!out || !d_mem || ((uintptr_t)d_mem & 255)) return BC_E_INVAL;
+    int rc = make_layout(h, L);
+    if (rc) return rc;
+    if (d_bytes < L.total) return BC_E_NOMEM;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    bc_index *ix = new (std::nothrow) bc_index();
+    if (!ix) return BC_E_NOMEM;
+    char *base = (char *)d_mem;
+    uint64_t n = h->fwd.n;
+    cudaError_t e = cudaSuccess;
+    for (int which = 0; which < 2 && e == cudaSuccess; ++which) {
+        const bc_bwt_host &b = which ? h->rev : h->fwd;
+        uint64_t *s_bwt = (uint64_t *)(base + L.off_stage_bwt);
+        uint32_t *s_occ = (uint32_t *)(base + L.off_stage_occ);
+        BcLine *lines = (BcLine *)(base + (which ? L.off_rev : L.off_fwd));
+        e = cudaMemcpyAsync(s_bwt, b.bwt2, (n / 32 + 1) * 8, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(s_occ, b.occ, (n / b.occ_interval + 1) * 16, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) {
+            unsigned grid = (unsigned)((L.n_lines + 255) / 256);
+            bc_relayout_kernel<<<grid, 256, 0, st>>>(s_bwt, s_occ, b.occ_interval, n, L.n_lines, lines);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // staging is reused; host arrays are borrowed
+        BcBwtDev &d = ix->dev.bwt[which];
+        d.lines = (const uint4 *)lines;
+        d.n = (uint32_t)n;
+        d.primary = (uint32_t)b.primary;
+        for (int c = 0; c < 4; ++c) d.C[c] = (uint32_t)b.C[c];
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(base + L.off_sa, h->sa, (n / h->sa_interval + 1) * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { delete ix; return BC_E_CUDA; }
+    ix->dev.sa = (const uint32_t *)(base + L.off_sa);
+    ix->dev.sa_interval = h->sa_interval;
+    ix->n = n;
+    ix->bytes = L.total;
+    ix->ctas_per_sm = 0; ix->warps_per_cta = 0;
+    for (int i = 0; i < 8; ++i) ix->stats[i] = 0;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete ix; return BC_E_CUDA;
+    }
+    ix->sm_count = sms;
+    *out = ix;
+    return BC_OK;
+}
+
+extern "C" int bc_index_free(bc_index *ix) {
+    if (!ix) return BC_E_INVAL;
+    delete ix;
+    return BC_OK;
+}
+
+extern "C" int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream) {
+    if (!ix || (n_rows && (!d_rows || !d_pos))) return BC_E_INVAL;
+    if (n_rows == 0) return BC_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint64_t grid = (n_rows + 255) / 256;
+    if (grid > 0x7FFFFFFFull) return BC_E_INVAL;
+    bc_locate_kernel<<<(unsigned)grid, 256, 0, st>>>(ix->dev, d_rows, n_rows, d_pos);
+    if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return BC_E_CUDA;
+    return BC_OK;
+}
+
+extern "C" int bc_last_stats(const bc_index *ix, uint64_t *out8) {
+    if (!ix || !out8) return BC_E_INVAL;
+    for (int i = 0; i < 8; ++i) out8[i] = ix->stats[i];
+    return BC_OK;
+}
+
+extern "C" int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta) {
+    if (!ix || warps_per_cta > 32 || ctas_per_sm > 32) return BC_E_INVAL;
+    ix->ctas_per_sm = ctas_per_sm;
+    ix->warps_per_cta = warps_per_cta;
+    return BC_OK;
+}
+
+extern "C" const char *bc_strerror(int s) {
+    switch (s) {
+        case BC_OK: return "ok";
+        case BC_E_INVAL: return "invalid argument";
+        case BC_E_NOMEM: return "caller-provided buffer too small";
+        case BC_E_CUDA: return "CUDA error";
+        case BC_E_OVERFLOW: return "hit arena or hits_capacity too small (see n_hits_needed)";
+        case BC_E_UNSUPPORTED: return "unsupported";
+        default: return "unknown status";
+    }
+}
