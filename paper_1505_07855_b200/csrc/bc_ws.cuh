@@ -1,0 +1,61 @@
+// Workspace layout and launch interfaces between bc_align.cu (host orchestration), bc_search.cu
+// (A1-A5) and bc_post.cu (A6).  Internal.
+#pragma once
+#include "bc_internal.cuh"
+
+// prepared query entry (uint16) for consumption step t of query q = 2*read + strand:
+//   bits 0-2  base consumed at step t (strand 1: complemented), 4 = N
+//   bits 3-8  D[t]  = lower bound on differences needed for W[t..m-1], clamped to 63
+//   bits 9-14 Ds[t] = same for the unconsumed seed part W[t..seed_len-1] (0 outside the seed)
+#define BC_PREP_BASE(p) ((p) & 7u)
+#define BC_PREP_D(p) (((p) >> 3) & 63u)
+#define BC_PREP_DS(p) (((p) >> 9) & 63u)
+
+enum {                      // indices into the uint64 counter block
+    BC_CTR_TICKET = 0,      // next query to hand to a warp
+    BC_CTR_ARENA = 1,       // raw hits produced (cursor; may exceed the capacity)
+    BC_CTR_NODES = 2,
+    BC_CTR_LOOKUPS = 3,
+    BC_CTR_LINES = 4,
+    BC_CTR_ERROR = 5,       // bit 0: bad read length, bit 1: pool overflow (must never happen)
+    BC_CTR_DLOOKUPS = 6,
+    BC_CTR_POOLMAX = 7,
+    BC_CTR_NBIG = 8,        // queries whose raw segment is sorted by a whole CTA
+    BC_CTR_TOTAL = 9,       // hits after dedup
+    BC_CTR_COUNT = 16
+};
+
+struct BcRawHit { uint32_t qid, k, l, d; };
+
+struct BcWorkspace {        // device pointers into the caller's workspace
+    uint16_t *prep;         // [nq][stride]
+    uint32_t stride;
+    uint32_t *qcnt;         // [nq] raw hits per query
+    uint32_t *qfill;        // [nq] scatter cursors, later: unique hits per query
+    uint64_t *seg_off;      // [nq+1] exclusive scan of qcnt
+    uint64_t *uoff;         // [nq+1] exclusive scan of unique counts
+    uint64_t *blk;          // scan block sums
+    uint32_t *big;          // [nq] list of big segments
+    uint64_t *ctr;          // [BC_CTR_COUNT]
+    BcRawHit *arena;        // [arena_cap]
+    uint64_t *seg_key;      // [arena_cap] (k<<32 | l), grouped by query
+    uint32_t *seg_d;        // [arena_cap]
+    uint64_t arena_cap;
+    uint32_t nq;
+};
+
+struct BcSearchParams {
+    BcIndexDev ix;
+    bc_reads reads;
+    bc_opts o;
+    BcWorkspace ws;
+    uint32_t pool_cap;      // entries per warp pool
+};
+
+// launchers (return cudaError_t of the launch)
+cudaError_t bc_launch_prepare(const BcSearchParams &p, cudaStream_t st);
+cudaError_t bc_launch_search(const BcSearchParams &p, int sm_count, uint32_t ctas_per_sm, uint32_t warps_per_cta,
+                             cudaStream_t st);
+cudaError_t bc_launch_post(const BcSearchParams &p, bc_result res, cudaStream_t st);
+// smem bytes one pool entry takes; used by the host to size pools
+#define BC_POOL_ENTRY_BYTES 24u
