@@ -84,6 +84,8 @@ typedef struct {
     const uint64_t *off;      /* [n_reads] first base of read r in the stream */
     const uint16_t *len;      /* [n_reads] 1..BC_MAX_READ_LEN */
     uint32_t n_reads;
+    uint32_t max_len;         /* caller-declared upper bound of len[] (sizes the per-query rows of the
+                                 workspace); a read longer than it -> BC_E_INVAL */
 } bc_reads;
 
 typedef struct { uint32_t k, l; uint8_t d, strand; uint16_t zero; } bc_hit;   /* 12 bytes */
@@ -134,8 +136,9 @@ int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint3
 
 /* Device-side counters of the last bc_align_batch on this index (HOST out array of 8 uint64):
  * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] 64-byte lines fetched,
- * [3] raw hits, [4] D-kernel lookups, [5] pool high-water mark, [6] search-kernel ns (0 if not
- * timed), [7] reserved. */
+ * [3] raw hits, [4] D-kernel lookups, [5] pool high-water mark, [6] search-kernel ns (CUDA events
+ * on the caller's stream around the persistent search kernel), [7] geometry used:
+ * ctas_per_sm << 32 | warps_per_cta << 16 | pool entries per warp. */
 int bc_last_stats(const bc_index *ix, uint64_t *out8);
 
 /* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM, warps per CTA. */

@@ -1,0 +1,380 @@
+"""Thin Python binding of the C-ABI library of include/barracuda_b200.h (same names).
+
+Argument marshalling only: every step of the hot path (D[] bounds, inexact search, hit emission,
+sort + dedup, locate) runs in the CUDA kernels of csrc/.  PyTorch provides device memory and
+streams, nothing else.  There is no CPU fallback: without the compiled library (and, for the
+compute calls, a CUDA device) everything here raises.
+
+Paper passages behind each call are cited in include/barracuda_b200.h; the readings of what the
+paper leaves open are in DESIGN.md.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+import os
+
+import numpy as np
+
+from . import _build
+
+BC_OK, BC_E_INVAL, BC_E_NOMEM, BC_E_CUDA, BC_E_OVERFLOW, BC_E_UNSUPPORTED = 0, -1, -2, -3, -4, -5
+BC_MAX_READ_LEN = 256
+
+HIT_DTYPE = np.dtype([("k", "<u4"), ("l", "<u4"), ("d", "u1"), ("strand", "u1"), ("zero", "<u2")])
+
+
+class bc_bwt_host(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("primary", C.c_uint64), ("bwt2", C.c_void_p), ("occ_interval", C.c_uint32),
+                ("occ", C.c_void_p), ("C", C.c_uint64 * 5)]
+
+
+class bc_index_host(C.Structure):
+    _fields_ = [("fwd", bc_bwt_host), ("rev", bc_bwt_host), ("sa_interval", C.c_uint32), ("sa", C.c_void_p)]
+
+
+class bc_opts(C.Structure):
+    _fields_ = [(f, C.c_int32) for f in ("z", "max_gap_open", "max_gap_ext", "seed_len", "seed_z", "indel_end_skip")]
+
+
+class bc_reads(C.Structure):
+    _fields_ = [("bases2", C.c_void_p), ("nmask", C.c_void_p), ("off", C.c_void_p), ("len", C.c_void_p),
+                ("n_reads", C.c_uint32), ("max_len", C.c_uint32)]
+
+
+class bc_result(C.Structure):
+    _fields_ = [("hit_offsets", C.c_void_p), ("hits", C.c_void_p), ("hits_capacity", C.c_uint64),
+                ("n_hits_needed", C.c_void_p)]
+
+
+class BcError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {strerror(status)} ({status})")
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Built in-tree with nvcc if missing or stale; raises otherwise."""
+    global _lib
+    if _lib is None:
+        so = _build.build()
+        if not os.path.exists(so):
+            raise ImportError("libbarracuda_b200.so is missing and could not be built; there is no CPU fallback")
+        L = C.CDLL(so)
+        vp, u32, u64, i32 = C.c_void_p, C.c_uint32, C.c_uint64, C.c_int
+        L.bc_index_device_bytes.argtypes = [C.POINTER(bc_index_host), C.POINTER(C.c_size_t)]
+        L.bc_index_upload.argtypes = [C.POINTER(bc_index_host), vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.bc_index_free.argtypes = [vp]
+        L.bc_align_workspace_bytes.argtypes = [vp, u32, u32, C.POINTER(bc_opts), u32, C.POINTER(C.c_size_t)]
+        L.bc_align_batch.argtypes = [vp, C.POINTER(bc_reads), C.POINTER(bc_opts), C.POINTER(bc_result), vp, C.c_size_t, vp]
+        L.bc_locate.argtypes = [vp, vp, u64, vp, vp]
+        L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 8)]
+        L.bc_set_geometry.argtypes = [vp, u32, u32]
+        L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
+        L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
+        L.bc_strerror.argtypes = [i32]
+        L.bc_strerror.restype = C.c_char_p
+        for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
+                  "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_index_build_host",
+                  "bc_index_host_free"):
+            getattr(L, f).restype = i32
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return lib().bc_strerror(status).decode()
+
+
+def _check(status: int, where: str):
+    if status != BC_OK:
+        raise BcError(status, where)
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1505_07855_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+    return torch
+
+
+def _stream_ptr(torch, stream):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def make_opts(o) -> bc_opts:
+    if isinstance(o, bc_opts):
+        return o
+    t = o.astuple() if hasattr(o, "astuple") else tuple(o)
+    return bc_opts(*[int(x) for x in t])
+
+
+# --------------------------------------------------------------------------------------------
+# host index (transport arrays)
+# --------------------------------------------------------------------------------------------
+class HostIndex:
+    """Owner of a bc_index_host built by bc_index_build_host (host memory, library-allocated)."""
+
+    def __init__(self, ptr):
+        self._p = ptr
+
+    @property
+    def struct(self) -> bc_index_host:
+        return self._p.contents
+
+    @property
+    def n(self) -> int:
+        return int(self.struct.fwd.n)
+
+    def arrays(self, which: int = 0):
+        """(bwt2 uint64[], occ uint32[][4], C[5], primary, occ_interval) views of the fwd/rev BWT."""
+        b = self.struct.rev if which else self.struct.fwd
+        n = int(b.n)
+        bwt2 = np.ctypeslib.as_array(C.cast(b.bwt2, C.POINTER(C.c_uint64)), shape=(n // 32 + 1,))
+        occ = np.ctypeslib.as_array(C.cast(b.occ, C.POINTER(C.c_uint32)), shape=(n // b.occ_interval + 1, 4))
+        return bwt2, occ, [int(x) for x in b.C], int(b.primary), int(b.occ_interval)
+
+    def sa_samples(self):
+        s = self.struct
+        cnt = self.n // s.sa_interval + 1
+        return np.ctypeslib.as_array(C.cast(s.sa, C.POINTER(C.c_uint32)), shape=(cnt,)), int(s.sa_interval)
+
+    def free(self):
+        if self._p is not None:
+            lib().bc_index_host_free(self._p)
+            self._p = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def bc_index_build_host(text: np.ndarray, occ_interval: int = 128, sa_interval: int = 32,
+                        n_threads: int | None = None) -> HostIndex:
+    """Suffix-sort T$ and reverse(T)$ on the host (untimed helper)."""
+    text = np.ascontiguousarray(text, dtype=np.uint8)
+    out = C.POINTER(bc_index_host)()
+    rc = lib().bc_index_build_host(text.ctypes.data_as(C.c_void_p), text.size, occ_interval, sa_interval,
+                                   n_threads or os.cpu_count() or 1, C.byref(out))
+    _check(rc, "bc_index_build_host")
+    return HostIndex(out)
+
+
+# --------------------------------------------------------------------------------------------
+# device index
+# --------------------------------------------------------------------------------------------
+class DeviceIndex:
+    """bc_index handle + the torch buffer that backs it."""
+
+    def __init__(self, handle, mem, n, device):
+        self._h, self.mem, self.n, self.device = handle, mem, n, device
+
+    @property
+    def handle(self):
+        if self._h is None:
+            raise RuntimeError("index was freed")
+        return self._h
+
+    def free(self):
+        if self._h is not None:
+            lib().bc_index_free(self._h)
+            self._h = None
+            self.mem = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def bc_index_device_bytes(h: HostIndex) -> int:
+    b = C.c_size_t(0)
+    _check(lib().bc_index_device_bytes(h._p, C.byref(b)), "bc_index_device_bytes")
+    return int(b.value)
+
+
+def bc_index_upload(h: HostIndex, device="cuda:0", stream=None) -> DeviceIndex:
+    """Index wholly resident in GPU memory, re-laid out as 64-byte rank lines."""
+    torch = _torch()
+    nbytes = bc_index_device_bytes(h)
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        mem = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        ptr = (mem.data_ptr() + 255) & ~255
+        out = C.c_void_p()
+        rc = lib().bc_index_upload(h._p, C.c_void_p(ptr), nbytes, _stream_ptr(torch, stream), C.byref(out))
+    _check(rc, "bc_index_upload")
+    return DeviceIndex(out, mem, h.n, dev)
+
+
+def bc_set_geometry(ix: DeviceIndex, ctas_per_sm: int = 0, warps_per_cta: int = 0):
+    _check(lib().bc_set_geometry(ix.handle, ctas_per_sm, warps_per_cta), "bc_set_geometry")
+
+
+STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry")
+
+
+def bc_last_stats(ix: DeviceIndex) -> dict:
+    a = (C.c_uint64 * 8)()
+    _check(lib().bc_last_stats(ix.handle, C.byref(a)), "bc_last_stats")
+    return dict(zip(STAT_NAMES, [int(x) for x in a]))
+
+
+# --------------------------------------------------------------------------------------------
+# reads and results
+# --------------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class DeviceReads:
+    """bc_reads with torch-owned device tensors (int-typed views of the unsigned transport arrays)."""
+    bases2: object      # int32 tensor  (uint32 words)
+    nmask: object       # int32 tensor or None
+    off: object         # int64 tensor  (uint64)
+    len: object         # int16 tensor  (uint16)
+    n_reads: int
+    max_len: int
+
+    def struct(self) -> bc_reads:
+        return bc_reads(self.bases2.data_ptr() if self.n_reads else None,
+                        self.nmask.data_ptr() if (self.nmask is not None and self.n_reads) else None,
+                        self.off.data_ptr() if self.n_reads else None,
+                        self.len.data_ptr() if self.n_reads else None, self.n_reads, self.max_len)
+
+
+class HostReads:
+    """Packed reads in pinned host memory (the transport layout of bc_reads)."""
+
+    def __init__(self, bases2: np.ndarray, nmask, off: np.ndarray, ln: np.ndarray, pin: bool = True):
+        import torch
+        self.n_reads = int(ln.size)
+        self.max_len = int(ln.max()) if ln.size else 1
+
+        def t(a, dt):
+            x = torch.from_numpy(np.ascontiguousarray(a).view(dt))
+            return x.pin_memory() if (pin and torch.cuda.is_available() and x.numel()) else x
+        self.bases2 = t(bases2.astype(np.uint32, copy=False), np.int32)
+        self.nmask = None if nmask is None else t(nmask.astype(np.uint32, copy=False), np.int32)
+        self.off = t(off.astype(np.uint64, copy=False), np.int64)
+        self.len = t(ln.astype(np.uint16, copy=False), np.int16)
+
+    @property
+    def nbytes(self) -> int:
+        ts = [self.bases2, self.off, self.len] + ([self.nmask] if self.nmask is not None else [])
+        return sum(x.numel() * x.element_size() for x in ts)
+
+    def to_device(self, device="cuda:0") -> DeviceReads:
+        _torch()
+        nm = None if self.nmask is None else self.nmask.to(device, non_blocking=True)
+        return DeviceReads(self.bases2.to(device, non_blocking=True), nm, self.off.to(device, non_blocking=True),
+                           self.len.to(device, non_blocking=True), self.n_reads, self.max_len)
+
+
+@dataclasses.dataclass
+class AlignResult:
+    hit_offsets: object     # int64 tensor [n_reads+1] (device)
+    hits: object            # uint8 tensor [n_hits*12] (device), records of HIT_DTYPE
+    n_hits: int
+    n_raw: int
+
+    def to_numpy(self):
+        """(hit_offsets uint64[n_reads+1], hits HIT_DTYPE[n_hits]) on the host."""
+        off = self.hit_offsets.cpu().numpy().view(np.uint64)
+        hits = self.hits[: self.n_hits * 12].cpu().numpy().view(HIT_DTYPE)
+        return off, hits
+
+
+class Workspace:
+    """Caller-owned device buffers of bc_align_batch, reusable across batches of the same shape."""
+
+    def __init__(self, ix: DeviceIndex, n_reads: int, max_len: int, opts, raw_hits_per_read: int = 16,
+                 hits_capacity: int | None = None):
+        torch = _torch()
+        self.ix, self.n_reads, self.max_len = ix, n_reads, max_len
+        self.opts = make_opts(opts)
+        b = C.c_size_t(0)
+        _check(lib().bc_align_workspace_bytes(ix.handle, n_reads, max_len, C.byref(self.opts), raw_hits_per_read,
+                                              C.byref(b)), "bc_align_workspace_bytes")
+        self.ws_bytes = int(b.value)
+        self.raw_hits_per_read = raw_hits_per_read
+        with torch.cuda.device(ix.device):
+            self.mem = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=ix.device)
+            self.hits_capacity = int(hits_capacity if hits_capacity is not None else max(1024, 4 * n_reads))
+            self.hit_offsets = torch.empty(n_reads + 1, dtype=torch.int64, device=ix.device)
+            self.hits = torch.empty(self.hits_capacity * 12, dtype=torch.uint8, device=ix.device)
+            self.needed = torch.zeros(2, dtype=torch.int64, device=ix.device)
+
+    @property
+    def ptr(self) -> int:
+        return (self.mem.data_ptr() + 255) & ~255
+
+
+def bc_align_workspace_bytes(ix: DeviceIndex, n_reads: int, max_len: int, opts, raw_hits_per_read: int = 0) -> int:
+    b = C.c_size_t(0)
+    o = make_opts(opts)
+    _check(lib().bc_align_workspace_bytes(ix.handle, n_reads, max_len, C.byref(o), raw_hits_per_read, C.byref(b)),
+           "bc_align_workspace_bytes")
+    return int(b.value)
+
+
+def bc_align_batch_raw(ix: DeviceIndex, reads: DeviceReads, opts, ws: Workspace, stream=None) -> int:
+    """One call of the C entry point; returns its status code (no retry, no exception)."""
+    torch = _torch()
+    o = make_opts(opts)
+    r = reads.struct()
+    res = bc_result(ws.hit_offsets.data_ptr(), ws.hits.data_ptr(), ws.hits_capacity, ws.needed.data_ptr())
+    with torch.cuda.device(ix.device):
+        return lib().bc_align_batch(ix.handle, C.byref(r), C.byref(o), C.byref(res), C.c_void_p(ws.ptr), ws.ws_bytes,
+                                    _stream_ptr(torch, stream))
+
+
+def bc_align_batch(ix: DeviceIndex, reads: DeviceReads, opts, ws: Workspace | None = None, stream=None,
+                   grow: bool = True):
+    """The hot path: per read, the deduplicated sorted SA intervals with
+    their minimum difference counts.  On BC_E_OVERFLOW the caller-owned buffers are re-allocated at
+    the size the library reports and the call is repeated (grow=True), else BcError is raised.
+    Returns (AlignResult, Workspace)."""
+    if ws is None:
+        ws = Workspace(ix, reads.n_reads, max(1, reads.max_len), opts)
+    for _ in range(4):
+        rc = bc_align_batch_raw(ix, reads, opts, ws, stream)
+        if rc == BC_OK:
+            need = ws.needed.cpu().numpy().view(np.uint64)
+            return AlignResult(ws.hit_offsets, ws.hits, int(need[0]), int(need[1])), ws
+        if rc != BC_E_OVERFLOW or not grow:
+            raise BcError(rc, "bc_align_batch")
+        need = ws.needed.cpu().numpy().view(np.uint64)
+        n_dedup, n_raw = int(need[0]), int(need[1])
+        per_read = max(ws.raw_hits_per_read, -(-n_raw // max(1, reads.n_reads)) + 1)
+        cap = max(ws.hits_capacity, n_dedup if n_dedup else ws.hits_capacity)
+        ws = Workspace(ix, reads.n_reads, max(1, reads.max_len), opts, per_read, cap)
+    raise BcError(BC_E_OVERFLOW, "bc_align_batch (after growing)")
+
+
+def bc_align_batch_host(ix: DeviceIndex, hreads: HostReads, opts, ws: Workspace | None = None, stream=None):
+    """End-to-end call with HOST buffers: pinned host reads -> device, bc_align_batch, CSR result
+    back to the host.  Returns (hit_offsets uint64[], hits HIT_DTYPE[], Workspace)."""
+    torch = _torch()
+    with torch.cuda.device(ix.device):
+        dreads = hreads.to_device(ix.device)
+        res, ws = bc_align_batch(ix, dreads, opts, ws, stream)
+        off, hits = res.to_numpy()
+    return off, hits, ws
+
+
+def bc_locate(ix: DeviceIndex, rows, stream=None):
+    """SA rows -> text coordinates: pos[i] = SA_fwd[rows[i]]."""
+    torch = _torch()
+    rows_t = torch.as_tensor(np.ascontiguousarray(rows, dtype=np.uint32).view(np.int32), device=ix.device) \
+        if not hasattr(rows, "data_ptr") else rows
+    pos = torch.empty_like(rows_t)
+    with torch.cuda.device(ix.device):
+        rc = lib().bc_locate(ix.handle, C.c_void_p(rows_t.data_ptr()), rows_t.numel(), C.c_void_p(pos.data_ptr()),
+                             _stream_ptr(torch, stream))
+    _check(rc, "bc_locate")
+    return pos

@@ -1,0 +1,162 @@
+// bc_align_batch / bc_align_workspace_bytes: host orchestration of the hot path.
+// Carves the caller's workspace, launches prepare -> search -> post on the caller's stream, reads
+// the counter block back and turns it into a status code.  No device allocation, no CPU fallback.
+#include "bc_ws.cuh"
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+constexpr uint64_t SCAN_TILE = 256 * 8;            // must match bc_post.cu
+constexpr size_t RAW_BYTES = sizeof(BcRawHit) + sizeof(uint64_t) + sizeof(uint32_t);   // arena + seg_key + seg_d
+
+struct WsLayout {
+    size_t off_prep, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_ctr, fixed;
+    uint32_t stride, nq;
+};
+
+int make_ws_layout(uint32_t n_reads, uint32_t max_len, WsLayout &L) {
+    if (max_len < 1 || max_len > BC_MAX_READ_LEN || n_reads > 0x7FFFFFF0u) return BC_E_INVAL;
+    L.nq = 2 * n_reads;
+    L.stride = (max_len + 2) & ~1u;                // max_len + 1 entries, even so rows stay 4-byte aligned
+    size_t o = 0;
+    L.off_prep = o;    o = align_up(o + (size_t)L.nq * L.stride * 2, 256);
+    L.off_qcnt = o;    o = align_up(o + (size_t)L.nq * 4, 256);
+    L.off_qfill = o;   o = align_up(o + (size_t)L.nq * 4, 256);
+    L.off_seg_off = o; o = align_up(o + ((size_t)L.nq + 1) * 8, 256);
+    L.off_uoff = o;    o = align_up(o + ((size_t)L.nq + 1) * 8, 256);
+    L.off_blk = o;     o = align_up(o + ((size_t)L.nq / SCAN_TILE + 2) * 8, 256);
+    L.off_big = o;     o = align_up(o + (size_t)L.nq * 4, 256);
+    L.off_ctr = o;     o = align_up(o + BC_CTR_COUNT * 8, 256);
+    L.fixed = o;
+    return BC_OK;
+}
+
+int check_opts(const bc_opts *o) {
+    if (!o) return BC_E_INVAL;
+    if (o->z < 0 || o->z > 255 || o->max_gap_open < 0 || o->max_gap_open > 255 || o->max_gap_ext < 0 ||
+        o->max_gap_ext > 255 || o->seed_len < 0 || o->seed_len > BC_MAX_READ_LEN || o->seed_z < 0 || o->seed_z > 255 ||
+        o->indel_end_skip < 0 || o->indel_end_skip > BC_MAX_READ_LEN)
+        return BC_E_INVAL;
+    return BC_OK;
+}
+
+}  // namespace
+
+extern "C" int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t max_len, const bc_opts *o,
+                                        uint32_t raw_hits_per_read, size_t *bytes) {
+    if (!ix || !bytes) return BC_E_INVAL;
+    int rc = check_opts(o);
+    if (rc) return rc;
+    WsLayout L;
+    rc = make_ws_layout(n_reads, max_len, L);
+    if (rc) return rc;
+    if (raw_hits_per_read == 0) raw_hits_per_read = 16;
+    uint64_t cap = (uint64_t)raw_hits_per_read * n_reads + 1024;
+    *bytes = L.fixed + 3 * 256 + cap * RAW_BYTES;
+    return BC_OK;
+}
+
+extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const bc_opts *o, bc_result *res,
+                              void *d_workspace, size_t ws_bytes, void *cuda_stream) {
+    bc_index *ix = const_cast<bc_index *>(ix_c);    // statistics live in the handle
+    if (!ix || !reads || !res || !d_workspace || ((uintptr_t)d_workspace & 255)) return BC_E_INVAL;
+    int rc = check_opts(o);
+    if (rc) return rc;
+    if (!res->hit_offsets || !res->n_hits_needed || (res->hits_capacity && !res->hits)) return BC_E_INVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    for (int i = 0; i < 8; ++i) ix->stats[i] = 0;
+    if (reads->n_reads == 0) {
+        uint64_t zero[3] = {0, 0, 0};
+        if (cudaMemcpyAsync(res->hit_offsets, zero, 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+            cudaMemcpyAsync(res->n_hits_needed, zero + 1, 16, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess)
+            return BC_E_CUDA;
+        return BC_OK;
+    }
+    if (!reads->bases2 || !reads->off || !reads->len) return BC_E_INVAL;
+    WsLayout L;
+    rc = make_ws_layout(reads->n_reads, reads->max_len, L);
+    if (rc) return rc;
+    if (ws_bytes < L.fixed + 3 * 256 + RAW_BYTES) return BC_E_NOMEM;
+
+    char *base = (char *)d_workspace;
+    BcSearchParams p;
+    p.ix = ix->dev;
+    p.reads = *reads;
+    p.o = *o;
+    BcWorkspace &ws = p.ws;
+    ws.nq = L.nq;
+    ws.stride = L.stride;
+    ws.prep = (uint16_t *)(base + L.off_prep);
+    ws.qcnt = (uint32_t *)(base + L.off_qcnt);
+    ws.qfill = (uint32_t *)(base + L.off_qfill);
+    ws.seg_off = (uint64_t *)(base + L.off_seg_off);
+    ws.uoff = (uint64_t *)(base + L.off_uoff);
+    ws.blk = (uint64_t *)(base + L.off_blk);
+    ws.big = (uint32_t *)(base + L.off_big);
+    ws.ctr = (uint64_t *)(base + L.off_ctr);
+    uint64_t cap = (ws_bytes - L.fixed - 3 * 256) / RAW_BYTES;
+    ws.arena_cap = cap;
+    size_t o_arena = L.fixed;
+    size_t o_key = align_up(o_arena + cap * sizeof(BcRawHit), 256);
+    size_t o_d = align_up(o_key + cap * sizeof(uint64_t), 256);
+    ws.arena = (BcRawHit *)(base + o_arena);
+    ws.seg_key = (uint64_t *)(base + o_key);
+    ws.seg_d = (uint32_t *)(base + o_d);
+
+    // geometry of the persistent kernel
+    uint32_t warps = ix->warps_per_cta ? ix->warps_per_cta : 8;
+    uint32_t ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 4;
+    const uint32_t R = 8u * (uint32_t)o->z + 9u;
+    size_t smem_budget = (size_t)(220 * 1024) / ctas;
+    if (smem_budget > 200 * 1024) smem_budget = 200 * 1024;
+    uint32_t pool_cap = (uint32_t)(smem_budget / ((size_t)warps * BC_POOL_ENTRY_BYTES));
+    if (pool_cap > 2048) pool_cap = 2048;
+    while (pool_cap < R + 16 && ctas > 1) {         // deep budgets need room: fewer CTAs per SM
+        --ctas;
+        smem_budget = (size_t)(220 * 1024) / ctas;
+        if (smem_budget > 200 * 1024) smem_budget = 200 * 1024;
+        pool_cap = (uint32_t)(smem_budget / ((size_t)warps * BC_POOL_ENTRY_BYTES));
+    }
+    if (pool_cap < R + 16) return BC_E_UNSUPPORTED;  // z too large for the on-chip pool at this warp count
+    p.pool_cap = pool_cap;
+
+    cudaError_t e = cudaMemsetAsync(base + L.off_qcnt, 0, L.fixed - L.off_qcnt, st);   // qcnt .. ctr
+    if (e == cudaSuccess) e = bc_launch_prepare(p, st);
+    if (e == cudaSuccess && ix->ev[0]) e = cudaEventRecord(ix->ev[0], st);
+    if (e == cudaSuccess) e = bc_launch_search(p, ix->sm_count, ctas, warps, st);
+    if (e == cudaSuccess && ix->ev[1]) e = cudaEventRecord(ix->ev[1], st);
+    if (e == cudaSuccess) e = bc_launch_post(p, *res, st);
+    uint64_t ctr[BC_CTR_COUNT];
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctr, ws.ctr, sizeof(ctr), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { cudaGetLastError(); return BC_E_CUDA; }
+
+    float ms = 0.f;
+    if (ix->ev[0] && ix->ev[1] && cudaEventElapsedTime(&ms, ix->ev[0], ix->ev[1]) != cudaSuccess) { ms = 0.f; cudaGetLastError(); }
+    ix->stats[0] = ctr[BC_CTR_NODES];
+    ix->stats[1] = ctr[BC_CTR_LOOKUPS];
+    ix->stats[2] = ctr[BC_CTR_LINES];
+    ix->stats[3] = ctr[BC_CTR_ARENA];
+    ix->stats[4] = ctr[BC_CTR_DLOOKUPS];
+    ix->stats[5] = ctr[BC_CTR_POOLMAX];
+    ix->stats[6] = (uint64_t)((double)ms * 1e6);
+    ix->stats[7] = (uint64_t)ctas << 32 | (uint64_t)warps << 16 | pool_cap;
+
+    if (ctr[BC_CTR_ERROR] & 1ull) return BC_E_INVAL;        // a read length outside 1..max_len
+    if (ctr[BC_CTR_ERROR] & 2ull) return BC_E_CUDA;         // pool bound violated: a bug, never silent
+    uint64_t needed[2] = {ctr[BC_CTR_TOTAL], ctr[BC_CTR_ARENA]};
+    if (ctr[BC_CTR_ARENA] > cap) {
+        needed[0] = 0;
+        if (cudaMemcpyAsync(res->n_hits_needed, needed, 16, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess)
+            return BC_E_CUDA;
+        return BC_E_OVERFLOW;
+    }
+    if (cudaMemcpyAsync(res->n_hits_needed + 1, needed + 1, 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return BC_E_CUDA;
+    if (ctr[BC_CTR_TOTAL] > res->hits_capacity) return BC_E_OVERFLOW;
+    return BC_OK;
+}

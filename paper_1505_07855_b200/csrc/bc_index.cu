@@ -149,12 +149,18 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
         delete ix; return BC_E_CUDA;
     }
     ix->sm_count = sms;
+    ix->ev[0] = ix->ev[1] = nullptr;
+    if (cudaEventCreate(&ix->ev[0]) != cudaSuccess || cudaEventCreate(&ix->ev[1]) != cudaSuccess) {
+        if (ix->ev[0]) cudaEventDestroy(ix->ev[0]);
+        delete ix; return BC_E_CUDA;
+    }
     *out = ix;
     return BC_OK;
 }
 
 extern "C" int bc_index_free(bc_index *ix) {
     if (!ix) return BC_E_INVAL;
+    for (int i = 0; i < 2; ++i) if (ix->ev[i]) cudaEventDestroy(ix->ev[i]);
     delete ix;
     return BC_OK;
 }

@@ -42,6 +42,7 @@ struct bc_index {            // the opaque handle of the ABI
     uint32_t ctas_per_sm, warps_per_cta;
     uint64_t stats[8];
     int sm_count;
+    cudaEvent_t ev[2];       // around the search kernel of the last bc_align_batch (stats[6])
 };
 
 #ifdef __CUDACC__

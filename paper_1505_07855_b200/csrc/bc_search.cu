@@ -41,7 +41,7 @@ __global__ void bc_prepare_kernel(BcSearchParams p) {
     uint32_t r = q >> 1, strand = q & 1;
     uint32_t m = p.reads.len[r];
     uint16_t *out = p.ws.prep + (size_t)q * p.ws.stride;
-    if (m < 1 || m > BC_MAX_READ_LEN) {
+    if (m < 1 || m > p.reads.max_len) {
         atomicOr((unsigned long long *)&p.ws.ctr[BC_CTR_ERROR], 1ull);
         return;
     }
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(BC_SEARCH_THREADS, 2) bc_search_kernel(BcSearc
             if (ok) {
                 m = p.reads.len[q >> 1];
                 uint32_t pr = p.ws.prep[(size_t)q * p.ws.stride];
-                ok = m >= 1 && m <= BC_MAX_READ_LEN && (int)BC_PREP_D(pr) <= z && (int)BC_PREP_DS(pr) <= seed_z;
+                ok = m >= 1 && m <= p.reads.max_len && (int)BC_PREP_D(pr) <= z && (int)BC_PREP_DS(pr) <= seed_z;
             }
             uint32_t mask = __ballot_sync(0xffffffffu, ok);
             if (ok) {
