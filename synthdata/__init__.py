@@ -245,15 +245,8 @@ def make_reads(cfg: Config, genome: np.ndarray, first: int = 0, count: int | Non
     return Reads(out, anchor, strand)
 
 
-def pack_reads(codes: np.ndarray):
-    """Pack (n_reads, m) codes into the bc_reads transport layout.
-
-    Returns (bases2 uint32[], nmask uint32[], off uint64[n_reads], len uint16[n_reads]).
-    Base i of the stream sits at bits 2*(i%16) of bases2[i//16]; N -> code 0 and its nmask bit
-    (bit i%32 of nmask[i//32]) set.  Reads are concatenated without padding.
-    """
-    nr, m = codes.shape
-    flat = codes.reshape(-1)
+def _pack_stream(flat: np.ndarray):
+    """flat codes (0..3, 4 = N) -> (bases2 uint32[], nmask uint32[]) of the bc_reads transport layout."""
     total = flat.size
     isn = flat == 4
     two = np.where(isn, 0, flat).astype(np.uint32)
@@ -264,6 +257,18 @@ def pack_reads(codes: np.ndarray):
     padn = (-total) % 32
     nb = np.concatenate([isn.astype(np.uint32), np.zeros(padn, dtype=np.uint32)]).reshape(-1, 32)
     nmask = np.bitwise_or.reduce(nb << np.arange(32, dtype=np.uint32)[None, :], axis=1).astype(np.uint32)
+    return bases2, nmask
+
+
+def pack_reads(codes: np.ndarray):
+    """Pack (n_reads, m) codes into the bc_reads transport layout.
+
+    Returns (bases2 uint32[], nmask uint32[], off uint64[n_reads], len uint16[n_reads]).
+    Base i of the stream sits at bits 2*(i%16) of bases2[i//16]; N -> code 0 and its nmask bit
+    (bit i%32 of nmask[i//32]) set.  Reads are concatenated without padding.
+    """
+    nr, m = codes.shape
+    bases2, nmask = _pack_stream(codes.reshape(-1))
     off = (np.arange(nr, dtype=np.uint64) * np.uint64(m))
     ln = np.full(nr, m, dtype=np.uint16)
     return bases2, nmask, off, ln
@@ -274,7 +279,7 @@ def pack_ragged(reads: list):
     lens = np.asarray([len(r) for r in reads], dtype=np.int64)
     off = np.concatenate([[0], np.cumsum(lens)[:-1]]).astype(np.uint64) if len(reads) else np.zeros(0, np.uint64)
     flat = np.concatenate([np.asarray(r, dtype=np.uint8) for r in reads]) if len(reads) else np.zeros(0, np.uint8)
-    b2, nm, _, _ = pack_reads(flat.reshape(1, -1)) if flat.size else (np.zeros(0, np.uint32), np.zeros(0, np.uint32), None, None)
+    b2, nm = _pack_stream(flat) if flat.size else (np.zeros(0, np.uint32), np.zeros(0, np.uint32))
     return b2, nm, off, lens.astype(np.uint16)
 
 

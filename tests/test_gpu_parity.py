@@ -1,0 +1,215 @@
+"""GPU parity: the CUDA path, called through the C-ABI (via the thin binding), against the CPU
+oracle, element by element on the same seeded inputs.  Integer work => the bar is BIT-EXACT on
+hit_offsets and on every 12-byte hit record.  These tests FAIL (never skip, never fall back) if the
+compiled library is missing on a GPU box."""
+import ctypes as C
+import os
+
+import numpy as np
+import pytest
+
+import synthdata as sd
+import paper_1505_07855_b200 as bc
+from oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "worked_example.txt")
+
+
+class Pair:
+    """genome -> (oracle index, device index), both built from the same seeded genome."""
+
+    def __init__(self, T, sa_interval=32):
+        self.T = T
+        self.oracle = Oracle(T)
+        self.host = bc.bc_index_build_host(T, 128, sa_interval)
+        self.ix = bc.bc_index_upload(self.host)
+
+
+def gpu_align(ix, reads_list, opts, **kw):
+    b2, nm, off, ln = sd.pack_ragged(reads_list)
+    h = bc.HostReads(b2, nm, off, ln)
+    off_g, hits_g, ws = bc.bc_align_batch_host(ix, h, opts, **kw)
+    return off_g, hits_g
+
+
+def assert_same(ix, oracle, reads_list, opts):
+    off_o, hits_o = oracle.align(reads_list, tuple(opts))
+    off_g, hits_g = gpu_align(ix, reads_list, opts)
+    assert np.array_equal(off_g, off_o)
+    assert hits_g.tobytes() == hits_o.tobytes()
+    return off_o, hits_o
+
+
+_pairs = {}
+
+
+def pair_for(cfg_name, n):
+    key = (cfg_name, n)
+    if key not in _pairs:
+        cfg = sd.CONFIGS[cfg_name].scaled(n=n)
+        _pairs[key] = (cfg, Pair(sd.make_genome(cfg)))
+    return _pairs[key]
+
+
+# --------------------------------------------------------------------------------------------
+def test_library_loaded_is_in_tree():
+    so = bc._build.SO
+    assert os.path.exists(so) and os.path.dirname(so).endswith("paper_1505_07855_b200")
+    assert bc.lib() is not None
+
+
+def test_worked_example_through_the_gpu():
+    """SURVEY C6 P1 fixture (tests/golden/worked_example.txt) straight through bc_align_batch + bc_locate."""
+    T = None
+    hits = []
+    for line in open(GOLD):
+        line = line.strip()
+        if line.startswith("T "):
+            T = sd.encode(line.split()[1])
+        elif line.startswith("HIT "):
+            left, right = line[4:].split(":")
+            f = left.split()
+            z, go, ge, E, sl, sz = map(int, f[1:7])
+            want = []
+            if right.strip() != "-":
+                for rec in right.split(";"):
+                    v = rec.strip().split(",")
+                    pos = sorted(int(x) for x in v[4].split("|")) if len(v) > 4 else None
+                    want.append((int(v[0]), int(v[1]), int(v[2]), int(v[3]), pos))
+            hits.append((f[0], (z, go, ge, sl, sz, E), want))
+    p = Pair(T, sa_interval=4)
+    for read, opts, want in hits:
+        off, h = gpu_align(p.ix, [sd.encode(read)], opts)
+        got = [(int(x["strand"]), int(x["k"]), int(x["l"]), int(x["d"])) for x in h]
+        assert got == [w[:4] for w in want], (read, opts)
+        for (s, k, l, d, pos) in want:
+            if pos is not None:
+                rows = np.arange(k, l + 1, dtype=np.uint32)
+                got_pos = bc.bc_locate(p.ix, rows).cpu().numpy().view(np.uint32)
+                assert sorted(got_pos.tolist()) == pos
+
+
+def test_config1_full_size():
+    """configs[0] of BASELINE.json at full size: 1 Mbp, 10,000 x 36 bp, z=2 mismatches only."""
+    cfg, p = pair_for("1", sd.CONFIGS["1"].n)
+    reads = sd.make_reads(cfg, p.T)
+    off, hits = assert_same(p.ix, p.oracle, list(reads.codes), cfg.opts.astuple())
+    # sanity statistic (most reads match uniquely)
+    assert int(off[-1]) >= 0.9 * reads.n_reads
+
+
+@pytest.mark.parametrize("name,n,n_reads", [("2", 2_000_000, 1500), ("3", 3_000_000, 1500), ("4", 3_000_000, 1000),
+                                             ("5a", 1_000_000, 300), ("5b", 3_000_000, 1000)])
+def test_config_recipes_scaled(name, n, n_reads):
+    """Every config's recipe (repeats, error profile, paired ends, N, seed, gaps) at a genome size
+    the oracle finishes in seconds; spans many warps' worth of queries and a ragged tail."""
+    cfg, p = pair_for(name, n)
+    cfg = cfg.scaled(n_reads=n_reads)
+    reads = sd.make_reads(cfg, p.T, 0, n_reads)
+    assert_same(p.ix, p.oracle, list(reads.codes), cfg.opts.astuple())
+
+
+def test_ragged_lengths_and_N():
+    cfg, p = pair_for("3", 3_000_000)
+    reads = sd.make_reads(cfg.scaled(n_reads=600), p.T, 0, 600)
+    rng = np.random.default_rng(5)
+    rl = []
+    for i, r in enumerate(reads.codes):
+        m = int(rng.integers(1, reads.m + 1))
+        r = r[:m].copy()
+        if i % 7 == 0:
+            r[rng.integers(0, m)] = 4
+        rl.append(r)
+    rl.append(np.full(40, 4, np.uint8))                 # all N: no hits
+    rl.append(np.asarray([2], np.uint8))                # length 1
+    for opts in [(2, 1, 2, 0, 0, 3), (3, 1, 2, 20, 1, 5), (1, 0, 0, 0, 0, 0), (2, 2, 2, 0, 0, 0)]:
+        # E = 0 with a length-1 read makes "everything" align; keep those reads longer
+        rr = rl if opts[5] > 0 else [r for r in rl if len(r) >= 12]
+        assert_same(p.ix, p.oracle, rr, opts)
+
+
+def test_max_read_length_and_exact():
+    cfg, p = pair_for("2", 2_000_000)
+    rng = np.random.default_rng(9)
+    rl = []
+    for _ in range(64):
+        s = int(rng.integers(0, p.T.size - 256))
+        r = p.T[s:s + 256].copy()
+        for q in rng.integers(0, 256, size=2):
+            r[q] = (r[q] + 1) & 3
+        rl.append(r)
+    assert_same(p.ix, p.oracle, rl, (3, 1, 2, 32, 1, 5))
+    off, hits = assert_same(p.ix, p.oracle, [p.T[1000:1256].copy()], (0, 0, 0, 0, 0, 5))
+    assert int(off[-1]) == 1 and int(hits[0]["d"]) == 0 and int(hits[0]["strand"]) == 0
+    assert bc.bc_locate(p.ix, np.asarray([hits[0]["k"]], np.uint32)).cpu().numpy().view(np.uint32)[0] == 1000
+
+
+def test_empty_batch_and_invalid_arguments():
+    cfg, p = pair_for("1", sd.CONFIGS["1"].n)
+    off, hits = gpu_align(p.ix, [], (2, 0, 0, 0, 0, 5))
+    assert off.tolist() == [0] and hits.size == 0
+    reads = [p.T[10:46].copy()]
+    with pytest.raises(bc.BcError) as e:
+        gpu_align(p.ix, reads, (256, 0, 0, 0, 0, 5))
+    assert e.value.status == bc.BC_E_INVAL
+    with pytest.raises(bc.BcError) as e:
+        gpu_align(p.ix, reads, (2, -1, 0, 0, 0, 5))
+    assert e.value.status == bc.BC_E_INVAL
+    # a read longer than the declared max_len is an error, not a truncation
+    b2, nm, o, ln = sd.pack_ragged(reads)
+    h = bc.HostReads(b2, nm, o, ln)
+    d = h.to_device()
+    d.max_len = 20
+    ws = bc.Workspace(p.ix, 1, 20, (2, 0, 0, 0, 0, 5))
+    assert bc.bc_align_batch_raw(p.ix, d, (2, 0, 0, 0, 0, 5), ws) == bc.BC_E_INVAL
+
+
+def test_overflow_is_reported_never_truncated():
+    """Repeat-rich genome, loose budget: many hits.  Too-small arena / hits buffer => BC_E_OVERFLOW
+    with the needed sizes; growing to them gives the oracle's answer."""
+    cfg, p = pair_for("2", 2_000_000)
+    reads = list(sd.make_reads(cfg.scaled(n_reads=400), p.T, 0, 400).codes)
+    opts = cfg.opts.astuple()
+    off_o, hits_o = p.oracle.align(reads, opts)
+    b2, nm, o, ln = sd.pack_ragged(reads)
+    d = bc.HostReads(b2, nm, o, ln).to_device()
+    ws = bc.Workspace(p.ix, len(reads), 51, opts, raw_hits_per_read=1, hits_capacity=8)
+    rc = bc.bc_align_batch_raw(p.ix, d, opts, ws)
+    assert rc == bc.BC_E_OVERFLOW
+    need = ws.needed.cpu().numpy().view(np.uint64)
+    assert int(need[1]) >= hits_o.size
+    ws2 = bc.Workspace(p.ix, len(reads), 51, opts, raw_hits_per_read=int(need[1]) // len(reads) + 1, hits_capacity=8)
+    rc = bc.bc_align_batch_raw(p.ix, d, opts, ws2)
+    assert rc == bc.BC_E_OVERFLOW
+    need = ws2.needed.cpu().numpy().view(np.uint64)
+    assert int(need[0]) == hits_o.size
+    res, _ = bc.bc_align_batch(p.ix, d, opts, ws2)     # grows and repeats
+    off_g, hits_g = res.to_numpy()
+    assert np.array_equal(off_g, off_o) and hits_g.tobytes() == hits_o.tobytes()
+
+
+def test_locate_equals_suffix_array():
+    cfg, p = pair_for("2", 2_000_000)
+    SA = p.oracle.index(0)[0]
+    rng = np.random.default_rng(3)
+    rows = np.concatenate([rng.integers(0, p.T.size + 1, size=20000), [0, p.T.size, p.oracle.index(0)[3]]]).astype(np.uint32)
+    pos = bc.bc_locate(p.ix, rows).cpu().numpy().view(np.uint32)
+    assert np.array_equal(pos, SA[rows])
+
+
+def test_result_independent_of_kernel_geometry():
+    """Deterministic output whatever the scheduling: different CTA/warp geometry => identical bytes."""
+    cfg, p = pair_for("2", 2_000_000)
+    reads = list(sd.make_reads(cfg.scaled(n_reads=3000), p.T, 0, 3000).codes)
+    opts = cfg.opts.astuple()
+    outs = []
+    for geo in [(0, 0), (1, 4), (2, 16), (3, 1)]:
+        bc.bc_set_geometry(p.ix, *geo)
+        off, hits = gpu_align(p.ix, reads, opts)
+        outs.append((off.tobytes(), hits.tobytes()))
+    bc.bc_set_geometry(p.ix, 0, 0)
+    assert all(o == outs[0] for o in outs)
+    st = bc.bc_last_stats(p.ix)
+    assert st["nodes"] > 0 and st["lookups"] == 2 * st["nodes"] or st["lookups"] > 0
