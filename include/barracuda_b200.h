@@ -109,8 +109,9 @@ typedef struct bc_index bc_index;   /* opaque handle (host object holding device
 int bc_index_device_bytes(const bc_index_host *h, size_t *bytes);
 
 /* Copies the transport arrays to the device and re-lays them out (kernel) into 64-byte lines:
- * {uint32 cnt[4]; uint64 lo[3]; uint64 hi[3]} = occurrences of A,C,G,T before symbol 192*i and
- * the two bit-planes of symbols 192*i .. 192*i+191, so that one rank query O(.,j) for all four
+ * {uint32 cnt[4]; uint32 lo[4]; uint32 hi[4]; uint32 mid[4]} = occurrences of A,C,G,T before symbol
+ * 128*i, the two bit-planes of symbols 128*i .. 128*i+127 and byte-packed counts at every 32nd
+ * symbol inside the line, so that one rank query O(.,j) for all four
  * symbols reads exactly one line (north_star).  d_mem: DEVICE, 256-byte aligned,
  * >= bc_index_device_bytes, owned by the caller and must outlive the handle. */
 int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_bytes, void *cuda_stream, bc_index **out);
@@ -134,14 +135,16 @@ int bc_align_batch(const bc_index *ix, const bc_reads *reads, const bc_opts *o, 
  * a sampled row.  d_rows, d_pos: DEVICE.  rows[i] must be in [0, n]. */
 int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream);
 
-/* Device-side counters of the last bc_align_batch on this index (HOST out array of 8 uint64):
+/* Device-side counters of the last bc_align_batch on this index (HOST out array of 16 uint64):
  * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] 64-byte lines fetched,
  * [3] raw hits, [4] D-kernel lookups, [5] pool high-water mark, [6] search-kernel ns (CUDA events
  * on the caller's stream around the persistent search kernel), [7] geometry used:
- * ctas_per_sm << 32 | warps_per_cta << 16 | pool entries per warp. */
-int bc_last_stats(const bc_index *ix, uint64_t *out8);
+ * ctas_per_sm << 32 | warps_per_cta << 16 | pool entries per warp, [8] warp-level branch steps,
+ * [9] nodes expanded in branch steps, [10] warp-level chain iterations, [11] nodes expanded in
+ * chain iterations, [12..15] reserved. */
+int bc_last_stats(const bc_index *ix, uint64_t *out16);
 
-/* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM, warps per CTA. */
+/* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM (<= 8), warps per CTA (<= 8). */
 int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
 
 /* Host-side index construction for synthetic genomes (untimed helper): suffix sort

@@ -71,7 +71,7 @@ def lib():
         L.bc_align_workspace_bytes.argtypes = [vp, u32, u32, C.POINTER(bc_opts), u32, C.POINTER(C.c_size_t)]
         L.bc_align_batch.argtypes = [vp, C.POINTER(bc_reads), C.POINTER(bc_opts), C.POINTER(bc_result), vp, C.c_size_t, vp]
         L.bc_locate.argtypes = [vp, vp, u64, vp, vp]
-        L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 8)]
+        L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 16)]
         L.bc_set_geometry.argtypes = [vp, u32, u32]
         L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
@@ -218,11 +218,12 @@ def bc_set_geometry(ix: DeviceIndex, ctas_per_sm: int = 0, warps_per_cta: int = 
     _check(lib().bc_set_geometry(ix.handle, ctas_per_sm, warps_per_cta), "bc_set_geometry")
 
 
-STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry")
+STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry",
+              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes")
 
 
 def bc_last_stats(ix: DeviceIndex) -> dict:
-    a = (C.c_uint64 * 8)()
+    a = (C.c_uint64 * 16)()
     _check(lib().bc_last_stats(ix.handle, C.byref(a)), "bc_last_stats")
     return dict(zip(STAT_NAMES, [int(x) for x in a]))
 

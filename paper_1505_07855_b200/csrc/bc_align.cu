@@ -65,7 +65,7 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     if (rc) return rc;
     if (!res->hit_offsets || !res->n_hits_needed || (res->hits_capacity && !res->hits)) return BC_E_INVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    for (int i = 0; i < 8; ++i) ix->stats[i] = 0;
+    for (int i = 0; i < 16; ++i) ix->stats[i] = 0;
     if (reads->n_reads == 0) {
         uint64_t zero[3] = {0, 0, 0};
         if (cudaMemcpyAsync(res->hit_offsets, zero, 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
@@ -107,7 +107,7 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
 
     // geometry of the persistent kernel
     uint32_t warps = ix->warps_per_cta ? ix->warps_per_cta : 8;
-    uint32_t ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 4;
+    uint32_t ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
     const uint32_t R = 8u * (uint32_t)o->z + 9u;
     size_t smem_budget = (size_t)(220 * 1024) / ctas;
     if (smem_budget > 200 * 1024) smem_budget = 200 * 1024;
@@ -143,6 +143,10 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     ix->stats[5] = ctr[BC_CTR_POOLMAX];
     ix->stats[6] = (uint64_t)((double)ms * 1e6);
     ix->stats[7] = (uint64_t)ctas << 32 | (uint64_t)warps << 16 | pool_cap;
+    ix->stats[8] = ctr[BC_CTR_BSTEPS];
+    ix->stats[9] = ctr[BC_CTR_BNODES];
+    ix->stats[10] = ctr[BC_CTR_CSTEPS];
+    ix->stats[11] = ctr[BC_CTR_NODES] - ctr[BC_CTR_BNODES];
 
     if (ctr[BC_CTR_ERROR] & 1ull) return BC_E_INVAL;        // a read length outside 1..max_len
     if (ctr[BC_CTR_ERROR] & 2ull) return BC_E_CUDA;         // pool bound violated: a bug, never silent

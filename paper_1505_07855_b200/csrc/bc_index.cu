@@ -65,11 +65,15 @@ __global__ void bc_relayout_kernel(const uint64_t *__restrict__ bwt2, const uint
     }
     BcLine L;
     for (int c = 0; c < 4; ++c) L.cnt[c] = cnt[c];
-    for (int q = 0; q < 3; ++q) {
-        uint64_t w0 = s0 / 32 + 2 * q;
-        uint64_t x0 = w0 < n_words ? bwt2[w0] : 0, x1 = w0 + 1 < n_words ? bwt2[w0 + 1] : 0;
-        L.lo[q] = (uint64_t)compact_even(x0) | ((uint64_t)compact_even(x1) << 32);
-        L.hi[q] = (uint64_t)compact_even(x0 >> 1) | ((uint64_t)compact_even(x1 >> 1) << 32);
+    uint32_t in_line[4] = {0, 0, 0, 0};
+    for (int q = 0; q < 4; ++q) {
+        uint64_t w0 = s0 / 32 + q;
+        uint64_t x = w0 < n_words ? bwt2[w0] : 0;
+        uint32_t lo = compact_even(x), hi = compact_even(x >> 1);
+        L.lo[q] = lo; L.hi[q] = hi;
+        L.mid[q] = in_line[0] | (in_line[1] << 8) | (in_line[2] << 16) | (in_line[3] << 24);
+        uint32_t nt = __popc(lo & hi), nc = __popc(lo & ~hi), ng = __popc(hi & ~lo);
+        in_line[0] += 32 - nt - nc - ng; in_line[1] += nc; in_line[2] += ng; in_line[3] += nt;
     }
     out[i] = L;
 }
@@ -84,10 +88,8 @@ __global__ void bc_locate_kernel(BcIndexDev ix, const uint32_t *__restrict__ row
     if (j > b.n) { pos[i] = 0xFFFFFFFFu; return; }
     while (j % ix.sa_interval != 0 && j != b.primary) {
         uint32_t p = j - (j > b.primary ? 1u : 0u);           // index of B[j] in the '$'-less string
-        BcLineRegs L = bc_load_line(b.lines, p / BC_LINE_SYMS);
-        uint32_t r = p % BC_LINE_SYMS, c = bc_line_symbol(L, r), o[4];
-        bc_line_rank4(L, r, o);
-        j = b.C[c] + o[c] + 1;                                // C[c] + O(c, j), O counts B[0..j] inclusive
+        uint32_t c = bc_symbol(b.lines, p);
+        j = b.C[c] + bc_rank1(b.lines, p, c) + 1;             // C[c] + O(c, j), O counts B[0..j] inclusive
         ++steps;
     }
     pos[i] = (j == b.primary ? 0u : ix.sa[j / ix.sa_interval]) + steps;
@@ -143,7 +145,7 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
     ix->n = n;
     ix->bytes = L.total;
     ix->ctas_per_sm = 0; ix->warps_per_cta = 0;
-    for (int i = 0; i < 8; ++i) ix->stats[i] = 0;
+    for (int i = 0; i < 16; ++i) ix->stats[i] = 0;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
         delete ix; return BC_E_CUDA;
@@ -176,14 +178,14 @@ extern "C" int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_
     return BC_OK;
 }
 
-extern "C" int bc_last_stats(const bc_index *ix, uint64_t *out8) {
-    if (!ix || !out8) return BC_E_INVAL;
-    for (int i = 0; i < 8; ++i) out8[i] = ix->stats[i];
+extern "C" int bc_last_stats(const bc_index *ix, uint64_t *out16) {
+    if (!ix || !out16) return BC_E_INVAL;
+    for (int i = 0; i < 16; ++i) out16[i] = ix->stats[i];
     return BC_OK;
 }
 
 extern "C" int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta) {
-    if (!ix || warps_per_cta > 32 || ctas_per_sm > 32) return BC_E_INVAL;
+    if (!ix || warps_per_cta > 8 || ctas_per_sm > 8) return BC_E_INVAL;
     ix->ctas_per_sm = ctas_per_sm;
     ix->warps_per_cta = warps_per_cta;
     return BC_OK;

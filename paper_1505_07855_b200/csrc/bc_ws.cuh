@@ -22,6 +22,9 @@ enum {                      // indices into the uint64 counter block
     BC_CTR_POOLMAX = 7,
     BC_CTR_NBIG = 8,        // queries whose raw segment is sorted by a whole CTA
     BC_CTR_TOTAL = 9,       // hits after dedup
+    BC_CTR_BSTEPS = 10,     // warp-level branch steps
+    BC_CTR_BNODES = 11,     // states expanded in branch steps
+    BC_CTR_CSTEPS = 12,     // warp-level chain iterations
     BC_CTR_COUNT = 16
 };
 

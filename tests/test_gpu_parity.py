@@ -205,7 +205,7 @@ def test_result_independent_of_kernel_geometry():
     reads = list(sd.make_reads(cfg.scaled(n_reads=3000), p.T, 0, 3000).codes)
     opts = cfg.opts.astuple()
     outs = []
-    for geo in [(0, 0), (1, 4), (2, 16), (3, 1)]:
+    for geo in [(0, 0), (1, 4), (2, 8), (5, 1)]:
         bc.bc_set_geometry(p.ix, *geo)
         off, hits = gpu_align(p.ix, reads, opts)
         outs.append((off.tobytes(), hits.tobytes()))

@@ -57,7 +57,7 @@ def check_against_oracle(T, occ_interval, sa_interval):
     n = T.size
     h = bc.bc_index_build_host(T, occ_interval, sa_interval, 4)
     o = Oracle(T, nthreads=4)
-    assert bc.bc_index_device_bytes(h) > 2 * (n // 192 + 1) * 64
+    assert bc.bc_index_device_bytes(h) > 2 * (n // 128 + 1) * 64
     for which in (0, 1):
         SA, B, Cc, primary = o.index(which)
         bwt2, occ, Ch, prim_h, oi = h.arrays(which)
@@ -76,7 +76,7 @@ def check_against_oracle(T, occ_interval, sa_interval):
     h.free()
 
 
-@pytest.mark.parametrize("n,occ_interval,sa_interval", [(1, 32, 1), (5, 32, 4), (191, 64, 32), (192, 128, 32),
+@pytest.mark.parametrize("n,occ_interval,sa_interval", [(1, 32, 1), (5, 32, 4), (127, 64, 32), (128, 128, 32), (191, 64, 32), (192, 128, 32),
                                                          (193, 128, 7), (4096, 128, 32), (50_000, 128, 32)])
 def test_host_index_matches_naive_suffix_sort(n, occ_interval, sa_interval):
     T = (sd.hash_u64(77, 1, np.arange(n, dtype=np.uint64)) >> np.uint64(62)).astype(np.uint8)
