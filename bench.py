@@ -277,6 +277,12 @@ def run_ours(args):
                      "kernel_ms": k_s * 1e3, "kernel_share_of_step": k_s * 1e3 / (t_ms / args.steps),
                      "nodes_per_launch": stats["nodes"], "occ_lookups_per_s": stats["lookups"] / k_s if k_s else 0.0,
                      "lines_per_launch": stats["lines"],
+                     "branch_nodes": stats["branch_nodes"], "chain_nodes": stats["chain_nodes"],
+                     "lanes_per_branch_step": stats["branch_nodes"] / max(1, stats["branch_steps"]),
+                     "lanes_per_chain_step": stats["chain_nodes"] / max(1, stats["chain_steps"]),
+                     "pool_max": stats["pool_max"], "geometry": {"ctas_per_sm": stats["geometry"] >> 32,
+                                                                 "warps_per_cta": (stats["geometry"] >> 16) & 0xFFFF,
+                                                                 "pool_entries_per_warp": stats["geometry"] & 0xFFFF},
                      "note": "algorithmic bytes = 64 B x index lines the search must read (1 or 2 per node, "
                              "counted by the kernel); this workload's 10.7 MB index is L2-resident, so the HBM "
                              "random-sector bound does not bind it (DESIGN.md 'Rooflines')"},
