@@ -108,12 +108,12 @@ typedef struct bc_index bc_index;   /* opaque handle (host object holding device
  * staging for the transport arrays). */
 int bc_index_device_bytes(const bc_index_host *h, size_t *bytes);
 
-/* Copies the transport arrays to the device and re-lays them out (kernel) into 64-byte lines:
- * {uint32 cnt[4]; uint32 lo[4]; uint32 hi[4]; uint32 mid[4]} = occurrences of A,C,G,T before symbol
- * 128*i, the two bit-planes of symbols 128*i .. 128*i+127 and byte-packed counts at every 32nd
- * symbol inside the line, so that one rank query O(.,j) for all four
- * symbols reads exactly one line (north_star).  d_mem: DEVICE, 256-byte aligned,
- * >= bc_index_device_bytes, owned by the caller and must outlive the handle. */
+/* Copies the transport arrays to the device and re-lays them out (kernel) into 32-byte blocks of 64
+ * symbols, two per 64-byte line: {uint32 cnt[4]; uint32 lo[2]; uint32 hi[2]} = occurrences of A,C,G,T
+ * before symbol 64*i and the two bit-planes of symbols 64*i .. 64*i+63, so that one rank query O(.,j)
+ * for all four symbols is ONE aligned 256-bit load inside one 64-byte line (north_star).
+ * d_mem: DEVICE, 256-byte aligned, >= bc_index_device_bytes, owned by the caller and must outlive
+ * the handle. */
 int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_bytes, void *cuda_stream, bc_index **out);
 
 /* Frees the handle only; d_mem stays the caller's. */
@@ -136,7 +136,7 @@ int bc_align_batch(const bc_index *ix, const bc_reads *reads, const bc_opts *o, 
 int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream);
 
 /* Device-side counters of the last bc_align_batch on this index (HOST out array of 16 uint64):
- * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] 64-byte lines fetched,
+ * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] distinct 32-byte index blocks (sectors) fetched,
  * [3] raw hits, [4] D-kernel lookups, [5] pool high-water mark, [6] search-kernel ns (CUDA events
  * on the caller's stream around the persistent search kernel), [7] geometry used:
  * ctas_per_sm << 32 | warps_per_cta << 16 | pool entries per warp, [8] warp-level branch steps,

@@ -22,8 +22,8 @@ int make_layout(const bc_index_host *h, Layout &L) {
     if (!h || !h->sa || h->sa_interval == 0 || !check_bwt(h->fwd) || !check_bwt(h->rev) || h->fwd.n != h->rev.n)
         return BC_E_INVAL;
     uint64_t n = h->fwd.n;
-    L.n_lines = n / BC_LINE_SYMS + 1;
-    L.lines_bytes = align_up(L.n_lines * 64, 256);
+    L.n_lines = n / BC_BLOCK_SYMS + 1;               // 32-byte blocks
+    L.lines_bytes = align_up(L.n_lines * 32, 256);
     L.off_fwd = 0;
     L.off_rev = L.lines_bytes;
     L.off_sa = 2 * L.lines_bytes;
@@ -48,12 +48,12 @@ __device__ __forceinline__ uint32_t compact_even(uint64_t x) {
     return (uint32_t)x;
 }
 
-// A0: one thread per 64-byte line
+// A0: one thread per 32-byte block
 __global__ void bc_relayout_kernel(const uint64_t *__restrict__ bwt2, const uint32_t *__restrict__ occ,
-                                   uint32_t occ_interval, uint64_t n, uint64_t n_lines, BcLine *__restrict__ out) {
+                                   uint32_t occ_interval, uint64_t n, uint64_t n_lines, BcBlock *__restrict__ out) {
     uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_lines) return;
-    uint64_t s0 = i * BC_LINE_SYMS;                  // first symbol of the line (may be == n: empty tail line)
+    uint64_t s0 = i * BC_BLOCK_SYMS;                 // first symbol of the block (may be == n: empty tail block)
     uint64_t n_words = n / 32 + 1;
     uint64_t t = s0 / occ_interval;
     uint32_t cnt[4];
@@ -63,17 +63,13 @@ __global__ void bc_relayout_kernel(const uint64_t *__restrict__ bwt2, const uint
         uint32_t nt = __popcll(lo & hi), nc = __popcll(lo & ~hi), ng = __popcll(hi & ~lo);
         cnt[0] += 32 - nt - nc - ng; cnt[1] += nc; cnt[2] += ng; cnt[3] += nt;
     }
-    BcLine L;
+    BcBlock L;
     for (int c = 0; c < 4; ++c) L.cnt[c] = cnt[c];
-    uint32_t in_line[4] = {0, 0, 0, 0};
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < 2; ++q) {
         uint64_t w0 = s0 / 32 + q;
         uint64_t x = w0 < n_words ? bwt2[w0] : 0;
-        uint32_t lo = compact_even(x), hi = compact_even(x >> 1);
-        L.lo[q] = lo; L.hi[q] = hi;
-        L.mid[q] = in_line[0] | (in_line[1] << 8) | (in_line[2] << 16) | (in_line[3] << 24);
-        uint32_t nt = __popc(lo & hi), nc = __popc(lo & ~hi), ng = __popc(hi & ~lo);
-        in_line[0] += 32 - nt - nc - ng; in_line[1] += nc; in_line[2] += ng; in_line[3] += nt;
+        L.lo[q] = compact_even(x);
+        L.hi[q] = compact_even(x >> 1);
     }
     out[i] = L;
 }
@@ -122,7 +118,7 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
         const bc_bwt_host &b = which ? h->rev : h->fwd;
         uint64_t *s_bwt = (uint64_t *)(base + L.off_stage_bwt);
         uint32_t *s_occ = (uint32_t *)(base + L.off_stage_occ);
-        BcLine *lines = (BcLine *)(base + (which ? L.off_rev : L.off_fwd));
+        BcBlock *lines = (BcBlock *)(base + (which ? L.off_rev : L.off_fwd));
         e = cudaMemcpyAsync(s_bwt, b.bwt2, (n / 32 + 1) * 8, cudaMemcpyHostToDevice, st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(s_occ, b.occ, (n / b.occ_interval + 1) * 16, cudaMemcpyHostToDevice, st);
         if (e == cudaSuccess) {

@@ -7,27 +7,26 @@
 
 // ---------------------------------------------------------------------------------------------
 // Device index layout (north_star: "each rank query is one 64-byte line").
-// Line i of a BWT covers symbols 128*i .. 128*i+127 of the '$'-less BWT string:
-//   uint32 cnt[4]   occurrences of A,C,G,T before symbol 128*i
-//   uint32 lo[4]    bit s%32 of lo[s/32] = low  bit of the code of symbol 128*i+s
-//   uint32 hi[4]    ... high bit
-//   uint32 mid[4]   mid[w] = four packed bytes: occurrences of A,C,G,T in symbols [0, 32*w) of the
-//                   line (mid[0] = 0), so a rank query touches ONE 32-bit word of each bit-plane
-// Lines are 64-byte aligned: one rank query = one line = two 32-byte sectors; all four counts cost
-// three popc, one symbol's count costs one.  Footprint n/2 bytes per BWT.
+// The '$'-less BWT string is cut into 32-byte BLOCKS of 64 symbols; two blocks share a 64-byte line:
+//   uint32 cnt[4]   occurrences of A,C,G,T before symbol 64*i
+//   uint32 lo[2]    bit s of the 64-bit word lo = low  bit of the code of symbol 64*i+s
+//   uint32 hi[2]    ... high bit
+// A rank query O(.,j) reads ONE block = one aligned 32-byte sector with ONE 256-bit load
+// (LDG.E.256), i.e. half a line: all four counts cost three 64-bit popc, one symbol's count one.
+// Footprint n/2 bytes per BWT.  (Round-1 history: 192-symbol lines with 64-bit planes were ALU-bound,
+// 128-symbol lines read with four narrow loads were L1-request-bound; profiles/r01_*.)
 // ---------------------------------------------------------------------------------------------
-#define BC_LINE_SYMS 128u
+#define BC_BLOCK_SYMS 64u
 
-struct BcLine {
+struct BcBlock {
     uint32_t cnt[4];
-    uint32_t lo[4];
-    uint32_t hi[4];
-    uint32_t mid[4];
+    uint32_t lo[2];
+    uint32_t hi[2];
 };
-static_assert(sizeof(BcLine) == 64, "line must be 64 bytes");
+static_assert(sizeof(BcBlock) == 32, "block must be 32 bytes");
 
 struct BcBwtDev {
-    const uint4 *lines;      // n/128 + 1 lines, each 4 x uint4
+    const uint4 *lines;      // n/64 + 1 blocks of 2 x uint4 (32-byte aligned)
     uint32_t n;              // |T|
     uint32_t primary;        // row of '$'
     uint32_t C[4];           // C[c] = # symbols smaller than c
@@ -56,38 +55,47 @@ __device__ __forceinline__ uint32_t bc_rank_pos(const BcBwtDev &b, uint32_t x) {
     return x - (x > b.primary ? 1u : 0u);          // symbols of the '$'-less string before row x
 }
 
+struct BcBlockRegs { uint32_t c0, c1, c2, c3; uint64_t lo, hi; };
+
+// one 256-bit read-only load of the block that holds position p of the '$'-less string
+__device__ __forceinline__ BcBlockRegs bc_load_block(const uint4 *lines, uint32_t p) {
+    const uint4 *q = lines + (size_t)(p >> 6) * 2;
+    BcBlockRegs r;
+    uint32_t l0, l1, h0, h1;
+    asm("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
+        : "l"(q));
+    r.lo = ((uint64_t)l1 << 32) | l0;
+    r.hi = ((uint64_t)h1 << 32) | h0;
+    return r;
+}
+
 // all four O(., .) before position p of the '$'-less string: out[c] = #{j < p : B'[j] = c}
 __device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_t out[4]) {
-    const uint32_t *L = reinterpret_cast<const uint32_t *>(lines + (size_t)(p >> 7) * 4);
-    const uint32_t w = (p >> 5) & 3u, b = p & 31u;
-    const uint4 c = __ldg(reinterpret_cast<const uint4 *>(L));
-    uint32_t lo = __ldg(L + 4 + w), hi = __ldg(L + 8 + w);
-    const uint32_t mid = __ldg(L + 12 + w);
-    const uint32_t m = (1u << b) - 1u;
-    lo &= m; hi &= m;
-    const uint32_t nt = __popc(lo & hi), nc = __popc(lo & ~hi), ng = __popc(hi & ~lo);
-    out[0] = c.x + (mid & 255u) + (b - nc - ng - nt);
-    out[1] = c.y + ((mid >> 8) & 255u) + nc;
-    out[2] = c.z + ((mid >> 16) & 255u) + ng;
-    out[3] = c.w + (mid >> 24) + nt;
+    const BcBlockRegs r = bc_load_block(lines, p);
+    const uint32_t b = p & 63u;
+    const uint64_t m = (1ull << b) - 1ull;
+    const uint64_t lo = r.lo & m, hi = r.hi & m;
+    const uint32_t nt = __popcll(lo & hi), nc = __popcll(lo & ~hi), ng = __popcll(hi & ~lo);
+    out[0] = r.c0 + (b - nc - ng - nt);
+    out[1] = r.c1 + nc;
+    out[2] = r.c2 + ng;
+    out[3] = r.c3 + nt;
 }
 
 // one symbol's count: #{j < p : B'[j] = c}
 __device__ __forceinline__ uint32_t bc_rank1(const uint4 *lines, uint32_t p, uint32_t c) {
-    const uint32_t *L = reinterpret_cast<const uint32_t *>(lines + (size_t)(p >> 7) * 4);
-    const uint32_t w = (p >> 5) & 3u, b = p & 31u;
-    const uint32_t base = __ldg(L + c);
-    uint32_t lo = __ldg(L + 4 + w), hi = __ldg(L + 8 + w);
-    const uint32_t mid = __ldg(L + 12 + w);
-    lo = (c & 1u) ? lo : ~lo;
-    hi = (c & 2u) ? hi : ~hi;
-    return base + ((mid >> (8u * c)) & 255u) + __popc(lo & hi & ((1u << b) - 1u));
+    const BcBlockRegs r = bc_load_block(lines, p);
+    const uint32_t b = p & 63u;
+    const uint64_t lo = (c & 1u) ? r.lo : ~r.lo, hi = (c & 2u) ? r.hi : ~r.hi;
+    const uint32_t base = (c & 2u) ? ((c & 1u) ? r.c3 : r.c2) : ((c & 1u) ? r.c1 : r.c0);
+    return base + __popcll(lo & hi & ((1ull << b) - 1ull));
 }
 
 // symbol at position p of the '$'-less string
 __device__ __forceinline__ uint32_t bc_symbol(const uint4 *lines, uint32_t p) {
-    const uint32_t *L = reinterpret_cast<const uint32_t *>(lines + (size_t)(p >> 7) * 4);
-    const uint32_t w = (p >> 5) & 3u, b = p & 31u;
-    return ((__ldg(L + 4 + w) >> b) & 1u) | (((__ldg(L + 8 + w) >> b) & 1u) << 1);
+    const uint32_t *L = reinterpret_cast<const uint32_t *>(lines + (size_t)(p >> 6) * 2);
+    const uint32_t w = (p >> 5) & 1u, b = p & 31u;
+    return ((__ldg(L + 4 + w) >> b) & 1u) | (((__ldg(L + 6 + w) >> b) & 1u) << 1);
 }
 #endif

@@ -20,12 +20,12 @@ __device__ __forceinline__ uint32_t read_base(const bc_reads &rd, uint64_t pos) 
 }
 
 // all four O(., j) for the two ends of the row interval [k, k+s-1]: olo = O(., k-1), ohi = O(., k+s-1).
-// Returns the number of distinct 64-byte lines touched (1 or 2).
+// Returns the number of distinct 32-byte blocks (sectors) touched (1 or 2).
 __device__ __forceinline__ uint32_t rank4_pair(const BcBwtDev &b, uint32_t k, uint32_t s, uint32_t olo[4], uint32_t ohi[4]) {
     const uint32_t plo = bc_rank_pos(b, k), phi = bc_rank_pos(b, k + s);
     bc_rank4(b.lines, plo, olo);
     bc_rank4(b.lines, phi, ohi);
-    return 1u + ((plo >> 7) != (phi >> 7) ? 1u : 0u);
+    return 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcS
                         const BcBwtDev &X = p.ix.bwt[strand ? 0 : 1];
                         const uint32_t plo = bc_rank_pos(X, k), phi = bc_rank_pos(X, k + s);
                         const uint32_t olo = bc_rank1(X.lines, plo, c), ohi = bc_rank1(X.lines, phi, c);
-                        n_lines += 1u + ((plo >> 7) != (phi >> 7) ? 1u : 0u);
+                        n_lines += 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
                         if (ohi == olo) act = false;
                         else {
                             k = X.C[c] + olo + 1u; s = ohi - olo; ++t;
