@@ -280,7 +280,7 @@ def run_ours(args):
                      "branch_nodes": stats["branch_nodes"], "chain_nodes": stats["chain_nodes"],
                      "lanes_per_branch_step": stats["branch_nodes"] / max(1, stats["branch_steps"]),
                      "lanes_per_chain_step": stats["chain_nodes"] / max(1, stats["chain_steps"]),
-                     "pool_max": stats["pool_max"], "geometry": {"ctas_per_sm": stats["geometry"] >> 32,
+                     "pool_max": stats["pool_max"], "cancelled": stats["cancelled"], "spill_blocks": stats["spill_blocks"], "geometry": {"ctas_per_sm": stats["geometry"] >> 32,
                                                                  "warps_per_cta": (stats["geometry"] >> 16) & 0xFFFF,
                                                                  "pool_entries_per_warp": stats["geometry"] & 0xFFFF},
                      "note": "algorithmic bytes = 64 B x index lines the search must read (1 or 2 per node, "

@@ -119,8 +119,9 @@ int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_bytes, void *c
 /* Frees the handle only; d_mem stays the caller's. */
 int bc_index_free(bc_index *ix);
 
-/* Workspace bytes for a batch: fixed part (prepared queries with their D[] bounds, per-warp state
- * pools, counters) + a raw-hit arena of raw_hits_per_read * n_reads records (0 = default 16). */
+/* Workspace bytes for a batch: fixed part (prepared queries with their D[] bounds, the per-warp
+ * overflow area of the search kernel's state rings -- sized for the geometry set on the index when
+ * this is called -- and counters) + a raw-hit arena of raw_hits_per_read * n_reads records (0 = default 16). */
 int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t max_len, const bc_opts *o,
                              uint32_t raw_hits_per_read, size_t *bytes);
 
@@ -141,7 +142,9 @@ int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint3
  * on the caller's stream around the persistent search kernel), [7] geometry used:
  * ctas_per_sm << 32 | warps_per_cta << 16 | pool entries per warp, [8] warp-level branch steps,
  * [9] nodes expanded in branch steps, [10] warp-level chain iterations, [11] nodes expanded in
- * chain iterations, [12..15] reserved. */
+ * chain iterations, [12] branch states popped and put back because their children did not fit,
+ * [13] 32-entry blocks of branch states spilled from the on-chip rings to the workspace,
+ * [14..15] reserved. */
 int bc_last_stats(const bc_index *ix, uint64_t *out16);
 
 /* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM (<= 8), warps per CTA (<= 8). */

@@ -1,6 +1,8 @@
 // bc_align_batch / bc_align_workspace_bytes: host orchestration of the hot path.
 // Carves the caller's workspace, launches prepare -> search -> post on the caller's stream, reads
 // the counter block back and turns it into a status code.  No device allocation, no CPU fallback.
+#include <cstdlib>
+
 #include "bc_ws.cuh"
 
 namespace {
@@ -11,16 +13,17 @@ constexpr uint64_t SCAN_TILE = 256 * 8;            // must match bc_post.cu
 constexpr size_t RAW_BYTES = sizeof(BcRawHit) + sizeof(uint64_t) + sizeof(uint32_t);   // arena + seg_key + seg_d
 
 struct WsLayout {
-    size_t off_prep, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_ctr, fixed;
+    size_t off_prep, off_spill, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_ctr, fixed;
     uint32_t stride, nq;
 };
 
-int make_ws_layout(uint32_t n_reads, uint32_t max_len, WsLayout &L) {
+int make_ws_layout(uint32_t n_reads, uint32_t max_len, uint32_t grid_warps, WsLayout &L) {
     if (max_len < 1 || max_len > BC_MAX_READ_LEN || n_reads > 0x7FFFFFF0u) return BC_E_INVAL;
     L.nq = 2 * n_reads;
     L.stride = (max_len + 2) & ~1u;                // max_len + 1 entries, even so rows stay 4-byte aligned
     size_t o = 0;
     L.off_prep = o;    o = align_up(o + (size_t)L.nq * L.stride * 2, 256);
+    L.off_spill = o;   o = align_up(o + (size_t)grid_warps * BC_SPILL_BLOCKS * 32 * BC_POOL_ENTRY_BYTES, 256);
     L.off_qcnt = o;    o = align_up(o + (size_t)L.nq * 4, 256);
     L.off_qfill = o;   o = align_up(o + (size_t)L.nq * 4, 256);
     L.off_seg_off = o; o = align_up(o + ((size_t)L.nq + 1) * 8, 256);
@@ -30,6 +33,29 @@ int make_ws_layout(uint32_t n_reads, uint32_t max_len, WsLayout &L) {
     L.off_ctr = o;     o = align_up(o + BC_CTR_COUNT * 8, 256);
     L.fixed = o;
     return BC_OK;
+}
+
+struct Geometry { uint32_t ctas, warps, bcap, ccap; };
+
+// geometry of the persistent kernel: CTAs per SM, warps per CTA, per-warp branch ring (power of two)
+// and chain stack sizes that fill the shared memory of an SM
+int choose_geometry(const bc_index *ix, const bc_opts *o, Geometry &g) {
+    g.warps = ix->warps_per_cta ? ix->warps_per_cta : 8;
+    g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
+    const uint32_t R = 8u * (uint32_t)o->z + 9u;
+    for (;; --g.ctas) {
+        size_t total_kb = 160;                        // leaves ~64 KB of the SM's 228 KB to L1 (index sectors, prep rows)
+        if (const char *e = getenv("BC_SMEM_KB")) total_kb = (size_t)atoi(e);   // experiment knob
+        size_t budget = total_kb * 1024 / g.ctas;
+        if (budget > 200 * 1024) budget = 200 * 1024;
+        uint32_t per_warp = (uint32_t)(budget / ((size_t)g.warps * BC_POOL_ENTRY_BYTES));
+        if (per_warp > 4096) per_warp = 4096;
+        uint32_t bcap = 64;
+        while (bcap * 2 <= per_warp / 2) bcap *= 2;
+        while (bcap < 2 * R + 64 && bcap * 2 + 96 <= per_warp) bcap *= 2;     // deep budgets: a bigger ring
+        if (bcap >= R + 48 && per_warp >= bcap + 96) { g.bcap = bcap; g.ccap = per_warp - bcap; return BC_OK; }
+        if (g.ctas == 1) return BC_E_UNSUPPORTED;     // z too large for the on-chip pool at this warp count
+    }
 }
 
 int check_opts(const bc_opts *o) {
@@ -48,8 +74,11 @@ extern "C" int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, ui
     if (!ix || !bytes) return BC_E_INVAL;
     int rc = check_opts(o);
     if (rc) return rc;
+    Geometry g;
+    rc = choose_geometry(ix, o, g);
+    if (rc) return rc;
     WsLayout L;
-    rc = make_ws_layout(n_reads, max_len, L);
+    rc = make_ws_layout(n_reads, max_len, (uint32_t)ix->sm_count * g.ctas * g.warps, L);
     if (rc) return rc;
     if (raw_hits_per_read == 0) raw_hits_per_read = 16;
     uint64_t cap = (uint64_t)raw_hits_per_read * n_reads + 1024;
@@ -75,8 +104,11 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
         return BC_OK;
     }
     if (!reads->bases2 || !reads->off || !reads->len) return BC_E_INVAL;
+    Geometry g;
+    rc = choose_geometry(ix, o, g);
+    if (rc) return rc;
     WsLayout L;
-    rc = make_ws_layout(reads->n_reads, reads->max_len, L);
+    rc = make_ws_layout(reads->n_reads, reads->max_len, (uint32_t)ix->sm_count * g.ctas * g.warps, L);
     if (rc) return rc;
     if (ws_bytes < L.fixed + 3 * 256 + RAW_BYTES) return BC_E_NOMEM;
 
@@ -105,22 +137,11 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     ws.seg_key = (uint64_t *)(base + o_key);
     ws.seg_d = (uint32_t *)(base + o_d);
 
-    // geometry of the persistent kernel
-    uint32_t warps = ix->warps_per_cta ? ix->warps_per_cta : 8;
-    uint32_t ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
-    const uint32_t R = 8u * (uint32_t)o->z + 9u;
-    size_t smem_budget = (size_t)(220 * 1024) / ctas;
-    if (smem_budget > 200 * 1024) smem_budget = 200 * 1024;
-    uint32_t pool_cap = (uint32_t)(smem_budget / ((size_t)warps * BC_POOL_ENTRY_BYTES));
-    if (pool_cap > 2048) pool_cap = 2048;
-    while (pool_cap < R + 16 && ctas > 1) {         // deep budgets need room: fewer CTAs per SM
-        --ctas;
-        smem_budget = (size_t)(220 * 1024) / ctas;
-        if (smem_budget > 200 * 1024) smem_budget = 200 * 1024;
-        pool_cap = (uint32_t)(smem_budget / ((size_t)warps * BC_POOL_ENTRY_BYTES));
-    }
-    if (pool_cap < R + 16) return BC_E_UNSUPPORTED;  // z too large for the on-chip pool at this warp count
-    p.pool_cap = pool_cap;
+    const uint32_t ctas = g.ctas, warps = g.warps;
+    p.bcap = g.bcap;
+    p.ccap = g.ccap;
+    ws.spill = (uint2 *)(base + L.off_spill);
+    ws.spill_blocks = BC_SPILL_BLOCKS;
 
     cudaError_t e = cudaMemsetAsync(base + L.off_qcnt, 0, L.fixed - L.off_qcnt, st);   // qcnt .. ctr
     if (e == cudaSuccess) e = bc_launch_prepare(p, st);
@@ -142,11 +163,13 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     ix->stats[4] = ctr[BC_CTR_DLOOKUPS];
     ix->stats[5] = ctr[BC_CTR_POOLMAX];
     ix->stats[6] = (uint64_t)((double)ms * 1e6);
-    ix->stats[7] = (uint64_t)ctas << 32 | (uint64_t)warps << 16 | pool_cap;
+    ix->stats[7] = (uint64_t)ctas << 32 | (uint64_t)warps << 16 | (g.bcap + g.ccap);
     ix->stats[8] = ctr[BC_CTR_BSTEPS];
     ix->stats[9] = ctr[BC_CTR_BNODES];
     ix->stats[10] = ctr[BC_CTR_CSTEPS];
     ix->stats[11] = ctr[BC_CTR_NODES] - ctr[BC_CTR_BNODES];
+    ix->stats[12] = ctr[BC_CTR_CANCEL];
+    ix->stats[13] = ctr[BC_CTR_SPILL];
 
     if (ctr[BC_CTR_ERROR] & 1ull) return BC_E_INVAL;        // a read length outside 1..max_len
     if (ctr[BC_CTR_ERROR] & 2ull) return BC_E_CUDA;         // pool bound violated: a bug, never silent

@@ -83,13 +83,17 @@ __device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_
     out[3] = r.c3 + nt;
 }
 
-// one symbol's count: #{j < p : B'[j] = c}
-__device__ __forceinline__ uint32_t bc_rank1(const uint4 *lines, uint32_t p, uint32_t c) {
-    const BcBlockRegs r = bc_load_block(lines, p);
+// one symbol's count from a loaded block: #{j < p : B'[j] = c}  (c > 3 gives a don't-care value)
+__device__ __forceinline__ uint32_t bc_block_rank1(const BcBlockRegs &r, uint32_t p, uint32_t c) {
     const uint32_t b = p & 63u;
     const uint64_t lo = (c & 1u) ? r.lo : ~r.lo, hi = (c & 2u) ? r.hi : ~r.hi;
     const uint32_t base = (c & 2u) ? ((c & 1u) ? r.c3 : r.c2) : ((c & 1u) ? r.c1 : r.c0);
     return base + __popcll(lo & hi & ((1ull << b) - 1ull));
+}
+
+// one symbol's count: #{j < p : B'[j] = c}
+__device__ __forceinline__ uint32_t bc_rank1(const uint4 *lines, uint32_t p, uint32_t c) {
+    return bc_block_rank1(bc_load_block(lines, p), p, c);
 }
 
 // symbol at position p of the '$'-less string

@@ -19,15 +19,6 @@ __device__ __forceinline__ uint32_t read_base(const bc_reads &rd, uint64_t pos) 
     return c;
 }
 
-// all four O(., j) for the two ends of the row interval [k, k+s-1]: olo = O(., k-1), ohi = O(., k+s-1).
-// Returns the number of distinct 32-byte blocks (sectors) touched (1 or 2).
-__device__ __forceinline__ uint32_t rank4_pair(const BcBwtDev &b, uint32_t k, uint32_t s, uint32_t olo[4], uint32_t ohi[4]) {
-    const uint32_t plo = bc_rank_pos(b, k), phi = bc_rank_pos(b, k + s);
-    bc_rank4(b.lines, plo, olo);
-    bc_rank4(b.lines, phi, ohi);
-    return 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
-}
-
 // ---------------------------------------------------------------------------------------------
 // A1 + A2: one thread per query (read, strand).  SURVEY C7 loop, in W coordinates: pieces are
 // grown from W[m-1] leftwards by prepending on the opposite-direction index.
@@ -100,31 +91,36 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
     return (b & 2) ? hi : lo;
 }
 
-// pool entry, 6 words, stored field-major (SoA) per warp so that lanes hit distinct banks:
-//   qid | k | s | k2 | mlo | mhi
+// Pool entry = 24 bytes, array-of-structures, moved with three 64-bit shared-memory accesses:
+//   {qid, k} {s, k2} {mlo, mhi}
 //   mlo = t (bits 0-8) | st (9-10; 0 = M, 1 = I, 2 = D) | n_go (11-18) | n_ge (19-26)
 //   mhi = seed_d (0-7) | d (8-15) | m-1 (16-23)
 // One pool per warp holds two stacks: BRANCH states (budget left, d < z) grow up from slot 0,
-// CHAIN states (budget exhausted, d == z: only exact matching can follow) grow down from CAP-1.
+// Per warp: a RING of BRANCH states (budget left, d < z), whose cold bottom spills to global memory in
+// blocks of 32, and a stack of CHAIN states (budget exhausted, d == z: only exact matching follows).
 #define BC_SEARCH_MAX_THREADS 256
+#ifndef BC_SEARCH_MIN_CTAS
+#define BC_SEARCH_MIN_CTAS 3
+#endif
 
-struct WarpCtx {
-    uint32_t *P;
-    uint32_t CAP, lane, lt_mask;
-    unsigned long long *ctr;
-};
+__device__ __forceinline__ void ent_store(uint2 *P, uint32_t idx, uint32_t qid, uint32_t k, uint32_t s, uint32_t k2,
+                                          uint32_t mlo, uint32_t mhi) {
+    uint2 *e = P + idx * 3u;
+    e[0] = make_uint2(qid, k); e[1] = make_uint2(s, k2); e[2] = make_uint2(mlo, mhi);
+}
 
-// warp-aggregated append of raw hits (A5)
-__device__ __forceinline__ void emit_hits(BcRawHit *arena, unsigned long long arena_cap, uint32_t *qcnt, const WarpCtx &w,
-                                          bool emit, uint32_t qid, uint32_t kf, uint32_t s, uint32_t d) {
+// warp-aggregated append of raw hits (A5); called by all 32 lanes
+__device__ __noinline__ void emit_hits(BcRawHit *arena, unsigned long long arena_cap, uint32_t *qcnt,
+                                       unsigned long long *ctr, bool emit, uint32_t qid, uint32_t kf, uint32_t s, uint32_t d) {
+    const uint32_t lane = threadIdx.x & 31u;
     uint32_t emask = __ballot_sync(0xffffffffu, emit);
     if (emask == 0) return;
     unsigned long long base = 0;
     int leader = __ffs(emask) - 1;
-    if ((int)w.lane == leader) base = atomicAdd(&w.ctr[BC_CTR_ARENA], (unsigned long long)__popc(emask));
+    if ((int)lane == leader) base = atomicAdd(&ctr[BC_CTR_ARENA], (unsigned long long)__popc(emask));
     base = __shfl_sync(0xffffffffu, base, leader);
     if (emit) {
-        unsigned long long pos = base + __popc(emask & w.lt_mask);
+        unsigned long long pos = base + __popc(emask & ((1u << lane) - 1u));
         if (pos < arena_cap) arena[pos] = BcRawHit{qid, kf, kf + s - 1u, d};
         atomicAdd(&qcnt[qid], 1u);
     }
@@ -152,51 +148,146 @@ __device__ __noinline__ uint32_t replay_k2(const uint4 *lines, uint32_t primary,
     return k2;
 }
 
+struct SearchConsts {            // warp-uniform values the phases share; suffix = strand
+    const uint4 *lines0, *lines1;   // index the strand's query is matched on (strand 0: reverse index)
+    uint32_t primary0, primary1;
+    uint4 Cv0, Cv1;
+};
+
+// ---------------------------------------------------------------------------------------------
+// CHAIN phase (see the kernel's header comment).  Returns the number of parked chain states.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const SearchConsts &sc, uint2 *Cq,
+                                                uint32_t ccnt, bool must_finish, unsigned long long *ctr,
+                                                uint32_t &n_nodes, uint32_t &n_sect, uint32_t &n_steps) {
+    const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u;
+    bool act = false;
+    uint32_t qid = 0, k = 0, s = 0, k2 = 0, t = 0, m = 0, dz = 0;
+    uint32_t k0 = 0, s0 = 0, t0 = 0;                      // strand 0: the state k2 belongs to
+    const uint16_t *pp = p.ws.prep;
+    const uint4 *lines = sc.lines0;
+    uint32_t primary = 0;
+    uint4 Cv = sc.Cv0;
+    for (;;) {
+        const uint32_t idle = __ballot_sync(0xffffffffu, !act);
+        if (idle && ccnt) {
+            const uint32_t r = __popc(idle & lt_mask);
+            if (!act && r < ccnt) {
+                const uint2 *e = Cq + (ccnt - 1u - r) * 3u;
+                const uint2 a0 = e[0], a1 = e[1], a2 = e[2];
+                qid = a0.x; k = a0.y; s = a1.x; k2 = a1.y;
+                t = a2.x & 511u; m = ((a2.y >> 16) & 255u) + 1u; dz = (a2.y >> 8) & 255u;
+                k0 = k; s0 = s; t0 = t;
+                const uint32_t strand = qid & 1u;
+                pp = p.ws.prep + (size_t)qid * p.ws.stride;
+                lines = strand ? sc.lines1 : sc.lines0; primary = strand ? sc.primary1 : sc.primary0;
+                Cv = strand ? sc.Cv1 : sc.Cv0;
+                act = true;
+            }
+            const uint32_t take = __popc(idle);
+            ccnt -= take < ccnt ? take : ccnt;
+            __syncwarp();
+        }
+        const uint32_t am = __ballot_sync(0xffffffffu, act);
+        if (am == 0) return 0;
+        if (!must_finish && ccnt == 0 && __popc(am) < 16) break;      // park the survivors
+        n_nodes += __popc(am);
+        ++n_steps;
+        bool emit = false;
+        if (act) {
+            // the two index blocks do not depend on the base: issue all three loads together
+            const uint32_t x0 = k, x1 = k + s;
+            const uint32_t plo = x0 - (x0 > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
+            const BcBlockRegs rlo = bc_load_block(lines, plo), rhi = bc_load_block(lines, phi);
+            const uint32_t c = BC_PREP_BASE(pp[t]);
+            n_sect += 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
+            const uint32_t olo = bc_block_rank1(rlo, plo, c), ohi = bc_block_rank1(rhi, phi, c);
+            if (c > 3u || ohi == olo) act = false;
+            else {
+                k = sel4(Cv.x, Cv.y, Cv.z, Cv.w, c) + olo + 1u; s = ohi - olo; ++t;
+                if (t == m) { emit = true; act = false; }
+            }
+        }
+        if (__any_sync(0xffffffffu, emit)) {
+            uint32_t kf = k;
+            if (emit && !(qid & 1u)) kf = replay_k2(lines, primary, Cv, pp, k0, s0, k2, t0, t);
+            emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, kf, s, dz);
+        }
+    }
+    // park: strand 0 first brings k2 up to date
+    const uint32_t am = __ballot_sync(0xffffffffu, act);
+    if (act) {
+        if (!(qid & 1u) && t > t0) k2 = replay_k2(lines, primary, Cv, pp, k0, s0, k2, t0, t);
+        ent_store(Cq, __popc(am & lt_mask), qid, k, s, k2, t, (dz << 8) | ((m - 1u) << 16));
+    }
+    __syncwarp();
+    return __popc(am);
+}
+
 // ---------------------------------------------------------------------------------------------
 // A3 + A4 + A5.  Persistent kernel, one LIFO pool per warp, two kinds of step:
-//  * BRANCH step: the top `a` branch states are popped, one per lane, and expanded in lock step:
-//    all four child intervals from one rank4 pair (1-2 index lines) -> match, <=3 mismatch,
-//    <=4 deletion and 1 insertion children, pruned by the budgets and D/Ds.  Children that still
-//    have budget go back to the branch stack (match child deepest), children with d == z go to
-//    the chain stack, terminal children are emitted.
+//  * BRANCH step: up to 32 branch states are popped, one per lane, and expanded in lock step:
+//    all four child intervals from one rank4 pair (1-2 index sectors) -> match, <=3 mismatch,
+//    <=4 deletion and 1 insertion children, pruned by the budgets and D/Ds.  Every lane counts its
+//    surviving children, a warp scan assigns pool slots, and each lane writes its own children:
+//    those that still have budget to the branch stack (match child deepest), those with d == z to
+//    the chain stack; terminal children are emitted.
 //  * CHAIN phase: lanes pull chain states and extend them by exact matching only (one symbol's
 //    rank at both interval ends per step, no pool traffic), refilling from the chain stack as they
 //    die, until the stack is dry and fewer than half the lanes are busy; survivors are parked.
 // New queries are drawn from a global ticket counter whenever fewer than 32 branch states are
 // pending, so lanes stay busy and converged whatever the shape of the individual search trees.
-// Pool bound: with used = branch + chain entries, a = clamp((CAP - R - used)/8, .., 32)
-// and R = 8z+9; when that is < 1 the chain stack is drained first (it only shrinks), and a run of
-// single-state steps from height P never exceeds P-1+R because the match child is explored last.
+// Pool bound: a multi-lane step keeps only the leading lanes whose children leave the
+// ring at <= BCAP - R entries (R = 8z+9) and fit the chain stack; the others are un-popped.  Lane 0
+// alone may fill the ring up to BCAP, and a run of single-lane steps from height P <= BCAP - R never
+// exceeds P-1+R because the match child is explored last.  If even lane 0 does not fit, the chain
+// stack (which only shrinks) is drained first.  Spilling the ring's bottom to global memory is an
+// optimisation on top of that bound (it keeps steps 32 wide), not part of it.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcSearchParams p) {
-    extern __shared__ uint32_t pool_mem[];
-    WarpCtx w;
-    w.lane = threadIdx.x & 31u;
-    const uint32_t warp = threadIdx.x >> 5;
-    const uint32_t CAP = p.pool_cap;
-    w.CAP = CAP;
-    uint32_t *P = pool_mem + (size_t)warp * 6u * CAP;
-    w.P = P;
-    w.lt_mask = (1u << w.lane) - 1u;
-    const uint32_t lane = w.lane, lt_mask = w.lt_mask;
+__global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
+    extern __shared__ uint2 pool_mem[];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
+    uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
+    uint2 *Cq = P + 3u * BCAP;                                    // chain stack: slots 0 .. ccnt-1
+    uint2 *G = p.ws.spill + ((size_t)blockIdx.x * (blockDim.x >> 5) + warp) * ((size_t)p.ws.spill_blocks * 96u);
+    const uint32_t GB = p.ws.spill_blocks;
+    const uint32_t lt_mask = (1u << lane) - 1u;
     const int z = p.o.z, E = p.o.indel_end_skip, max_go = p.o.max_gap_open, max_ge = p.o.max_gap_ext;
     const int seed_len = p.o.seed_len, seed_z = p.o.seed_z;
-    const int R = 8 * z + 9;
+    const uint32_t R = 8u * (uint32_t)z + 9u;
     const uint32_t nq = p.ws.nq;
     const uint32_t full = p.ix.bwt[0].n + 1;
     unsigned long long *ctr = (unsigned long long *)p.ws.ctr;
-    w.ctr = ctr;
+    SearchConsts sc;
+    sc.lines0 = p.ix.bwt[1].lines; sc.lines1 = p.ix.bwt[0].lines;          // strand 0 searches the reverse index
+    sc.primary0 = p.ix.bwt[1].primary; sc.primary1 = p.ix.bwt[0].primary;
+    sc.Cv0 = make_uint4(p.ix.bwt[1].C[0], p.ix.bwt[1].C[1], p.ix.bwt[1].C[2], p.ix.bwt[1].C[3]);
+    sc.Cv1 = make_uint4(p.ix.bwt[0].C[0], p.ix.bwt[0].C[1], p.ix.bwt[0].C[2], p.ix.bwt[0].C[3]);
 
-    const uint4 *rv_lines = p.ix.bwt[1].lines;
-    const uint32_t rv_primary = p.ix.bwt[1].primary;
-    const uint4 rv_C = make_uint4(p.ix.bwt[1].C[0], p.ix.bwt[1].C[1], p.ix.bwt[1].C[2], p.ix.bwt[1].C[3]);
-    uint32_t bcnt = 0, ccnt = 0, pool_max = 0;
-    bool more = true;
-    unsigned long long n_nodes = 0, n_lines = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0;
+    uint32_t bb = 1u << 24, bcnt = 0, ccnt = 0, gsp = 0, pool_max = 0;   // ring bottom, counts, spilled blocks
+    bool more = true, force_drain = false;
+    unsigned long long n_nodes = 0, n_sect = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0, n_cancel = 0, n_spill = 0;
 
     for (;;) {
+        // ---- ring <-> global: keep the hot top of the branch stack on chip --------------------------
+        while (bcnt >= 64u && bcnt + 96u + R > BCAP && gsp < GB) {          // spill the bottom 32 entries
+            const uint2 *src = P + ((bb + lane) & BM) * 3u;
+            uint2 *dst = G + ((size_t)gsp * 32u + lane) * 3u;
+            dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+            bb += 32u; bcnt -= 32u; ++gsp; ++n_spill;
+            __syncwarp();
+        }
+        if (bcnt < 32u && gsp > 0u) {                                          // bring the last block back
+            --gsp; bb -= 32u;
+            const uint2 *src = G + ((size_t)gsp * 32u + lane) * 3u;
+            uint2 *dst = P + ((bb + lane) & BM) * 3u;
+            dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+            bcnt += 32u;
+            __syncwarp();
+        }
         // ---- intake: new root states while the branch stack is shallow ------------------------
-        if (more && bcnt < 32u && bcnt + ccnt + 40u <= CAP) {
+        if (more && bcnt < 32u && gsp == 0u && ccnt + 32u <= CCAP) {
             uint32_t need = 32u - bcnt;
             unsigned long long tk = 0;
             if (lane == 0) tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
@@ -213,9 +304,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcS
             uint32_t mask = __ballot_sync(0xffffffffu, ok);
             if (ok) {
                 uint32_t r = __popc(mask & lt_mask);
-                uint32_t pos = z > 0 ? bcnt + r : CAP - 1u - ccnt - r;
-                P[0 * CAP + pos] = (uint32_t)q; P[1 * CAP + pos] = 0; P[2 * CAP + pos] = full;
-                P[3 * CAP + pos] = 0; P[4 * CAP + pos] = 0; P[5 * CAP + pos] = (m - 1) << 16;
+                if (z > 0) ent_store(P, (bb + bcnt + r) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
+                else ent_store(Cq, ccnt + r, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
             }
             if (z > 0) bcnt += __popc(mask); else ccnt += __popc(mask);
             __syncwarp();
@@ -223,86 +313,24 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcS
         if (bcnt == 0 && ccnt == 0) { if (!more) break; continue; }
         pool_max = bcnt + ccnt > pool_max ? bcnt + ccnt : pool_max;
 
-        int a = ((int)CAP - R - (int)(bcnt + ccnt)) / 8;
-        if (ccnt > 0 && (ccnt >= 32u || bcnt == 0 || a < 1)) {
-            // ==== CHAIN phase ====================================================================
-            const bool must_finish = (bcnt == 0 && !more) || a < 1;   // a < 1: the drain must make room
-            bool act = false;
-            uint32_t qid = 0, k = 0, s = 0, k2 = 0, t = 0, m = 0, dz = 0;
-            uint32_t k0 = 0, s0 = 0, t0 = 0;                      // strand 0: state k2 belongs to
-            for (;;) {
-                uint32_t idle = __ballot_sync(0xffffffffu, !act);
-                if (idle && ccnt) {
-                    uint32_t r = __popc(idle & lt_mask);
-                    if (!act && r < ccnt) {
-                        uint32_t idx = CAP - ccnt + r;
-                        qid = P[0 * CAP + idx]; k = P[1 * CAP + idx]; s = P[2 * CAP + idx]; k2 = P[3 * CAP + idx];
-                        uint32_t mlo = P[4 * CAP + idx], mhi = P[5 * CAP + idx];
-                        t = mlo & 511u; m = ((mhi >> 16) & 255u) + 1u; dz = (mhi >> 8) & 255u;
-                        k0 = k; s0 = s; t0 = t;
-                        act = true;
-                    }
-                    uint32_t take = __popc(idle);
-                    ccnt -= take < ccnt ? take : ccnt;
-                    __syncwarp();
-                }
-                uint32_t am = __ballot_sync(0xffffffffu, act);
-                if (am == 0) break;
-                if (!must_finish && ccnt == 0 && __popc(am) < 16) {
-                    // park the survivors (strand 0 first brings k2 up to date)
-                    if (act) {
-                        if (!(qid & 1u) && t > t0) k2 = replay_k2(rv_lines, rv_primary, rv_C, p.ws.prep + (size_t)qid * p.ws.stride, k0, s0, k2, t0, t);
-                        uint32_t idx = CAP - 1u - __popc(am & lt_mask);
-                        P[0 * CAP + idx] = qid; P[1 * CAP + idx] = k; P[2 * CAP + idx] = s; P[3 * CAP + idx] = k2;
-                        P[4 * CAP + idx] = t; P[5 * CAP + idx] = (dz << 8) | ((m - 1u) << 16);
-                    }
-                    ccnt = __popc(am);
-                    __syncwarp();
-                    break;
-                }
-                n_nodes += (unsigned long long)__popc(am);
-                ++n_csteps;
-                bool emit = false;
-                if (act) {
-                    const uint32_t strand = qid & 1u;
-                    const uint32_t c = BC_PREP_BASE(p.ws.prep[(size_t)qid * p.ws.stride + t]);
-                    if (c > 3u) act = false;
-                    else {
-                        const BcBwtDev &X = p.ix.bwt[strand ? 0 : 1];
-                        const uint32_t plo = bc_rank_pos(X, k), phi = bc_rank_pos(X, k + s);
-                        const uint32_t olo = bc_rank1(X.lines, plo, c), ohi = bc_rank1(X.lines, phi, c);
-                        n_lines += 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
-                        if (ohi == olo) act = false;
-                        else {
-                            k = X.C[c] + olo + 1u; s = ohi - olo; ++t;
-                            if (t == m) { emit = true; act = false; }
-                        }
-                    }
-                }
-                if (__any_sync(0xffffffffu, emit)) {
-                    uint32_t kf = k;
-                    if (emit && !(qid & 1u)) kf = replay_k2(rv_lines, rv_primary, rv_C, p.ws.prep + (size_t)qid * p.ws.stride, k0, s0, k2, t0, t);
-                    emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, w, emit, qid, kf, s, dz);
-                }
-            }
+        if (ccnt > 0 && (ccnt >= 32u || bcnt == 0 || force_drain)) {
+            uint32_t nn = 0, ns_ = 0, st_ = 0;
+            ccnt = chain_phase(p, sc, Cq, ccnt, (bcnt == 0 && gsp == 0 && !more) || force_drain, ctr, nn, ns_, st_);
+            force_drain = false;
+            n_nodes += nn; n_sect += ns_; n_csteps += st_;
             continue;
         }
 
         // ==== BRANCH step ========================================================================
-        a = a < 1 ? 1 : (a > 32 ? 32 : a);
-        a = a > (int)bcnt ? (int)bcnt : a;
-        const bool act = (int)lane < a;
+        const uint32_t a = bcnt < 32u ? bcnt : 32u;
+        bool act = lane < a;
         uint32_t qid = 0, k = 0, s = 0, k2 = 0, mlo = 0, mhi = 0;
         if (act) {
-            uint32_t idx = bcnt - 1u - lane;
-            qid = P[0 * CAP + idx]; k = P[1 * CAP + idx]; s = P[2 * CAP + idx];
-            k2 = P[3 * CAP + idx]; mlo = P[4 * CAP + idx]; mhi = P[5 * CAP + idx];
+            const uint2 *e = P + ((bb + bcnt - 1u - lane) & BM) * 3u;
+            const uint2 a0 = e[0], a1 = e[1], a2 = e[2];
+            qid = a0.x; k = a0.y; s = a1.x; k2 = a1.y; mlo = a2.x; mhi = a2.y;
         }
         __syncwarp();
-        bcnt -= (uint32_t)a;
-        n_nodes += (unsigned long long)a;
-        n_bnodes += (unsigned long long)a;
-        ++n_bsteps;
 
         const int t = mlo & 511, st = (mlo >> 9) & 3, go = (mlo >> 11) & 255, ge = (mlo >> 19) & 255;
         const int sd = mhi & 255, d = (mhi >> 8) & 255, m = (int)((mhi >> 16) & 255) + 1;
@@ -320,12 +348,19 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcS
         const uint32_t qb = BC_PREP_BASE(pr0);
         uint32_t nk[4] = {0, 0, 0, 0}, ns[4] = {0, 0, 0, 0}, nk2[4] = {0, 0, 0, 0};
         if (has_base || del_ok) {
-            const BcBwtDev &X = p.ix.bwt[strand ? 0 : 1];
+            const uint4 *lines = strand ? sc.lines1 : sc.lines0;
+            const uint32_t primary = strand ? sc.primary1 : sc.primary0;
+            const uint4 Cv = strand ? sc.Cv1 : sc.Cv0;
+            const uint32_t x1 = k + s;
+            const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             uint32_t olo[4], ohi[4];
-            n_lines += rank4_pair(X, k, s, olo, ohi);
+            bc_rank4(lines, plo, olo);
+            bc_rank4(lines, phi, ohi);
+            n_sect += 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
+            const uint32_t Cc[4] = {Cv.x, Cv.y, Cv.z, Cv.w};
             uint32_t acc = k2 + s;                       // k2 + dollar + prefix, built below
 #pragma unroll
-            for (int b = 0; b < 4; ++b) { ns[b] = ohi[b] - olo[b]; nk[b] = X.C[b] + olo[b] + 1u; acc -= ns[b]; }
+            for (int b = 0; b < 4; ++b) { ns[b] = ohi[b] - olo[b]; nk[b] = Cc[b] + olo[b] + 1u; acc -= ns[b]; }
 #pragma unroll
             for (int b = 0; b < 4; ++b) { nk2[b] = acc; acc += ns[b]; }
         }
@@ -352,62 +387,110 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcS
         const bool term_base = (int)tn == m;             // children that consume W[t] finish the read
         const bool term_del = t == m;
 
+        // child bit masks: bit 0 match; 1-4 mismatch with symbol bit-1; 5-8 deletion of symbol bit-5; 9 insertion
+        uint32_t vbits = 0;
 #pragma unroll
-        for (int slot = 0; slot < 10; ++slot) {
-            // slot 0: match; 1-4: mismatch with symbol slot-1; 5-8: deletion of symbol slot-5; 9: insertion
-            bool valid, terminal, chain;
-            uint32_t ck = k, cs = s, ck2 = k2, clo, chi;
-            if (slot == 0) {
-                ck = sel4(nk[0], nk[1], nk[2], nk[3], qb); cs = sel4(ns[0], ns[1], ns[2], ns[3], qb);
-                ck2 = sel4(nk2[0], nk2[1], nk2[2], nk2[3], qb);
-                valid = has_base && qb < 4u && cs > 0u; terminal = term_base; chain = false;
-                clo = ma_lo; chi = ma_hi;
-            } else if (slot <= 4) {
-                const int b = slot - 1;
-                ck = nk[b]; cs = ns[b]; ck2 = nk2[b];
-                valid = v_mm && qb != (uint32_t)b && cs > 0u; terminal = term_base; chain = last1;
-                clo = ma_lo; chi = mm_hi;
-            } else if (slot <= 8) {
-                const int b = slot - 5;
-                ck = nk[b]; cs = ns[b]; ck2 = nk2[b];
-                valid = v_del && cs > 0u; terminal = term_del; chain = last1;
-                clo = de_lo; chi = de_hi;
-            } else {
-                valid = v_ins; terminal = term_base; chain = last1;
-                clo = in_lo; chi = mm_hi;
+        for (int b = 0; b < 4; ++b) {
+            const bool ne = ns[b] > 0u;
+            if (has_base && qb == (uint32_t)b && ne) vbits |= 1u;
+            if (v_mm && qb != (uint32_t)b && ne) vbits |= 2u << b;
+            if (v_del && ne) vbits |= 32u << b;
+        }
+        if (v_ins) vbits |= 512u;
+        const uint32_t tbits = (term_base ? 0x21Fu : 0u) | (term_del ? 0x1E0u : 0u);   // terminal children
+        uint32_t ebits = vbits & tbits;
+        if (s == full) ebits &= ~512u;                   // the empty string is not a hit (C3)
+        // a terminal state is expanded further only for trailing deletions (E == 0) with budget left
+        const uint32_t keep_t = E == 0 ? (last1 ? 1u : 0x3FFu) : 0u;
+        uint32_t pbits = vbits & (~tbits | keep_t);
+        uint32_t cbits = last1 ? (pbits & 0x3FEu) : 0u;
+
+        // slots: warp scan of (branch pushes | chain pushes << 16); net growth decides who is kept
+        const uint32_t mine = (uint32_t)__popc(pbits & ~cbits) | ((uint32_t)__popc(cbits) << 16);
+        uint32_t incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((int)lane >= o) incl += v;
+        }
+        // lanes 0..lane kept, the lanes behind un-popped: ring and chain occupancy after the step
+        const uint32_t ring_if = bcnt - (lane + 1u) + (incl & 0xFFFFu);
+        const uint32_t chain_if = ccnt + (incl >> 16);
+        const bool fits = act && ring_if + R <= BCAP && chain_if <= CCAP;
+        uint32_t keepmask = __ballot_sync(0xffffffffu, fits);
+        uint32_t akeep = keepmask == 0xffffffffu ? 32u : (uint32_t)(__ffs(~keepmask) - 1);   // leading run
+        if (akeep > a) akeep = a;
+        if (akeep == 0) {                                 // lane 0 alone may use the whole ring
+            const uint32_t r0 = __shfl_sync(0xffffffffu, ring_if, 0), c0 = __shfl_sync(0xffffffffu, chain_if, 0);
+            if (r0 <= BCAP && c0 <= CCAP) akeep = 1;
+        }
+        if (akeep == 0) {
+            if (ccnt == 0) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // cannot happen (pool bound)
+            force_drain = true;                           // nothing popped; make room first
+            n_cancel += a;
+            continue;
+        }
+        if (lane >= akeep) { act = false; pbits = 0; cbits = 0; ebits = 0; }
+        n_cancel += a - akeep;
+        const uint32_t tot = __shfl_sync(0xffffffffu, incl, akeep - 1u);
+        const uint32_t excl = incl - mine;
+        uint32_t bpos = bb + bcnt - akeep + (excl & 0xFFFFu);         // ring index (masked at the store)
+        uint32_t cpos = ccnt + (excl >> 16);
+        bcnt = bcnt - akeep + (tot & 0xFFFFu);
+        ccnt += tot >> 16;
+        n_nodes += akeep; n_bnodes += akeep; ++n_bsteps;
+
+        if (pbits) {
+            if (pbits & 1u) {
+                ent_store(P, (bpos++) & BM, qid, sel4(nk[0], nk[1], nk[2], nk[3], qb), sel4(ns[0], ns[1], ns[2], ns[3], qb),
+                          sel4(nk2[0], nk2[1], nk2[2], nk2[3], qb), ma_lo, ma_hi);
             }
-            const bool emit = valid && terminal && cs != full;
-            // a terminal state is expanded further only for trailing deletions (E == 0) with budget left
-            const bool push = valid && (!terminal || (E == 0 && !chain));
-            if (__any_sync(0xffffffffu, emit))
-                emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, w, emit, qid, strand ? ck : ck2, cs, (chi >> 8) & 255u);
-            const uint32_t bmask = __ballot_sync(0xffffffffu, push && !chain);
-            const uint32_t cmask = __ballot_sync(0xffffffffu, push && chain);
-            const bool room = bcnt + ccnt + (uint32_t)a <= CAP;   // always true (pool bound); never write outside
-            if (push && room) {
-                const uint32_t pos = chain ? CAP - 1u - ccnt - __popc(cmask & lt_mask) : bcnt + __popc(bmask & lt_mask);
-                P[0 * CAP + pos] = qid; P[1 * CAP + pos] = ck; P[2 * CAP + pos] = cs; P[3 * CAP + pos] = ck2;
-                P[4 * CAP + pos] = clo; P[5 * CAP + pos] = chi;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                if (pbits & (2u << b)) {
+                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], ma_lo, mm_hi);
+                    else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], ma_lo, mm_hi);
+                }
             }
-            if (!room && (bmask | cmask)) {                       // cannot happen; never silent
-                if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull);
-            } else {
-                bcnt += __popc(bmask);
-                ccnt += __popc(cmask);
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                if (pbits & (32u << b)) {
+                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], de_lo, de_hi);
+                    else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], de_lo, de_hi);
+                }
+            }
+            if (pbits & 512u) {
+                if (last1) ent_store(Cq, cpos++, qid, k, s, k2, in_lo, mm_hi);
+                else ent_store(P, (bpos++) & BM, qid, k, s, k2, in_lo, mm_hi);
+            }
+        }
+        if (__any_sync(0xffffffffu, ebits != 0u)) {
+#pragma unroll 1
+            for (int slot = 0; slot < 10; ++slot) {
+                const bool em = (ebits >> slot) & 1u;
+                if (!__any_sync(0xffffffffu, em)) continue;
+                const uint32_t b = slot == 0 ? qb : (uint32_t)((slot - 1) & 3);
+                uint32_t ck = sel4(nk[0], nk[1], nk[2], nk[3], b), cs = sel4(ns[0], ns[1], ns[2], ns[3], b);
+                uint32_t ck2 = sel4(nk2[0], nk2[1], nk2[2], nk2[3], b);
+                if (slot == 9) { ck = k; cs = s; ck2 = k2; }
+                emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, em, qid, strand ? ck : ck2, cs,
+                          (uint32_t)(slot == 0 ? d : nd1));
             }
         }
         __syncwarp();
     }
     // per-warp statistics
-    for (int o = 16; o > 0; o >>= 1) n_lines += __shfl_down_sync(0xffffffffu, n_lines, o);
+    for (int o = 16; o > 0; o >>= 1) n_sect += __shfl_down_sync(0xffffffffu, n_sect, o);
     if (lane == 0) {
         atomicAdd(&ctr[BC_CTR_NODES], n_nodes);
         atomicAdd(&ctr[BC_CTR_LOOKUPS], 2ull * n_nodes);
-        atomicAdd(&ctr[BC_CTR_LINES], n_lines);
+        atomicAdd(&ctr[BC_CTR_LINES], n_sect);
         atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
         atomicAdd(&ctr[BC_CTR_BSTEPS], n_bsteps);
         atomicAdd(&ctr[BC_CTR_BNODES], n_bnodes);
         atomicAdd(&ctr[BC_CTR_CSTEPS], n_csteps);
+        atomicAdd(&ctr[BC_CTR_CANCEL], n_cancel);
+        atomicAdd(&ctr[BC_CTR_SPILL], n_spill);
     }
 }
 
@@ -416,7 +499,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, 3) bc_search_kernel(BcS
 cudaError_t bc_launch_search(const BcSearchParams &p, int sm_count, uint32_t ctas_per_sm, uint32_t warps_per_cta,
                              cudaStream_t st) {
     if (p.ws.nq == 0) return cudaSuccess;
-    size_t smem = (size_t)warps_per_cta * p.pool_cap * BC_POOL_ENTRY_BYTES;
+    size_t smem = (size_t)warps_per_cta * (p.bcap + p.ccap) * BC_POOL_ENTRY_BYTES;
     cudaError_t e = cudaFuncSetAttribute(bc_search_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     bc_search_kernel<<<sm_count * ctas_per_sm, warps_per_cta * 32, smem, st>>>(p);

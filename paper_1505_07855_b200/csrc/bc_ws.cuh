@@ -25,6 +25,8 @@ enum {                      // indices into the uint64 counter block
     BC_CTR_BSTEPS = 10,     // warp-level branch steps
     BC_CTR_BNODES = 11,     // states expanded in branch steps
     BC_CTR_CSTEPS = 12,     // warp-level chain iterations
+    BC_CTR_CANCEL = 13,     // branch states popped and put back because their children did not fit
+    BC_CTR_SPILL = 14,      // 32-entry blocks moved from the branch rings to global memory
     BC_CTR_COUNT = 16
 };
 
@@ -44,6 +46,8 @@ struct BcWorkspace {        // device pointers into the caller's workspace
     uint64_t *seg_key;      // [arena_cap] (k<<32 | l), grouped by query
     uint32_t *seg_d;        // [arena_cap]
     uint64_t arena_cap;
+    uint2 *spill;           // [warps in the grid][spill_blocks][32 entries][3] overflow of the branch rings
+    uint32_t spill_blocks;  // blocks of 32 entries per warp
     uint32_t nq;
 };
 
@@ -52,7 +56,8 @@ struct BcSearchParams {
     bc_reads reads;
     bc_opts o;
     BcWorkspace ws;
-    uint32_t pool_cap;      // entries per warp pool
+    uint32_t bcap;          // branch ring entries per warp (power of two)
+    uint32_t ccap;          // chain stack entries per warp
 };
 
 // launchers (return cudaError_t of the launch)
@@ -62,3 +67,4 @@ cudaError_t bc_launch_search(const BcSearchParams &p, int sm_count, uint32_t cta
 cudaError_t bc_launch_post(const BcSearchParams &p, bc_result res, cudaStream_t st);
 // smem bytes one pool entry takes; used by the host to size pools
 #define BC_POOL_ENTRY_BYTES 24u
+#define BC_SPILL_BLOCKS 128u          // per warp: 128 x 32 entries x 24 B = 96 KB of workspace
