@@ -148,6 +148,25 @@ __device__ __noinline__ uint32_t replay_k2(const uint4 *lines, uint32_t primary,
     return k2;
 }
 
+// per-warp statistics: n_xsect is per lane (second sectors of a rank pair), the rest warp-uniform
+__device__ __noinline__ void flush_stats(unsigned long long *ctr, uint32_t lane, uint32_t n_cnodes, uint32_t n_xsect,
+                                         uint32_t n_bsteps, uint32_t n_bnodes, uint32_t n_csteps, uint32_t n_cancel,
+                                         uint32_t n_spill) {
+    uint32_t x = n_xsect;
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    if (lane == 0) {
+        const unsigned long long nodes = (unsigned long long)n_cnodes + n_bnodes;
+        atomicAdd(&ctr[BC_CTR_NODES], nodes);
+        atomicAdd(&ctr[BC_CTR_LOOKUPS], 2ull * nodes);
+        atomicAdd(&ctr[BC_CTR_LINES], nodes + x);          // one sector per node + the pairs that straddle two
+        atomicAdd(&ctr[BC_CTR_BSTEPS], (unsigned long long)n_bsteps);
+        atomicAdd(&ctr[BC_CTR_BNODES], (unsigned long long)n_bnodes);
+        atomicAdd(&ctr[BC_CTR_CSTEPS], (unsigned long long)n_csteps);
+        atomicAdd(&ctr[BC_CTR_CANCEL], (unsigned long long)n_cancel);
+        atomicAdd(&ctr[BC_CTR_SPILL], (unsigned long long)n_spill);
+    }
+}
+
 struct SearchConsts {            // warp-uniform values the phases share; suffix = strand
     const uint4 *lines0, *lines1;   // index the strand's query is matched on (strand 0: reverse index)
     uint32_t primary0, primary1;
@@ -157,17 +176,16 @@ struct SearchConsts {            // warp-uniform values the phases share; suffix
 // ---------------------------------------------------------------------------------------------
 // CHAIN phase (see the kernel's header comment).  Returns the number of parked chain states.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const SearchConsts &sc, uint2 *Cq,
-                                                uint32_t ccnt, bool must_finish, unsigned long long *ctr,
+__device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const SearchConsts &sc, const uint32_t *Ctab,
+                                                uint2 *Cq, uint32_t ccnt, bool must_finish, unsigned long long *ctr,
                                                 uint32_t &n_nodes, uint32_t &n_sect, uint32_t &n_steps) {
     const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u;
     bool act = false;
-    uint32_t qid = 0, k = 0, s = 0, k2 = 0, t = 0, m = 0, dz = 0;
+    uint32_t qid = 0, k = 0, s = 0, k2 = 0, t = 0, m = 0, dz = 0, c = 0;
     uint32_t k0 = 0, s0 = 0, t0 = 0;                      // strand 0: the state k2 belongs to
     const uint16_t *pp = p.ws.prep;
     const uint4 *lines = sc.lines0;
     uint32_t primary = 0;
-    uint4 Cv = sc.Cv0;
     for (;;) {
         const uint32_t idle = __ballot_sync(0xffffffffu, !act);
         if (idle && ccnt) {
@@ -176,12 +194,12 @@ __device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const S
                 const uint2 *e = Cq + (ccnt - 1u - r) * 3u;
                 const uint2 a0 = e[0], a1 = e[1], a2 = e[2];
                 qid = a0.x; k = a0.y; s = a1.x; k2 = a1.y;
-                t = a2.x & 511u; m = ((a2.y >> 16) & 255u) + 1u; dz = (a2.y >> 8) & 255u;
+                t = a2.x & 511u; c = a2.x >> 27;          // the entry carries the base W[t] (strand-adjusted)
+                m = ((a2.y >> 16) & 255u) + 1u; dz = (a2.y >> 8) & 255u;
                 k0 = k; s0 = s; t0 = t;
                 const uint32_t strand = qid & 1u;
                 pp = p.ws.prep + (size_t)qid * p.ws.stride;
                 lines = strand ? sc.lines1 : sc.lines0; primary = strand ? sc.primary1 : sc.primary0;
-                Cv = strand ? sc.Cv1 : sc.Cv0;
                 act = true;
             }
             const uint32_t take = __popc(idle);
@@ -195,30 +213,32 @@ __device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const S
         ++n_steps;
         bool emit = false;
         if (act) {
-            // the two index blocks do not depend on the base: issue all three loads together
             const uint32_t x0 = k, x1 = k + s;
             const uint32_t plo = x0 - (x0 > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
-            const BcBlockRegs rlo = bc_load_block(lines, plo), rhi = bc_load_block(lines, phi);
-            const uint32_t c = BC_PREP_BASE(pp[t]);
-            n_sect += 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
+            const bool two = (plo >> 6) != (phi >> 6);
+            const BcBlockRegs rlo = bc_load_block(lines, plo);
+            BcBlockRegs rhi = rlo;
+            if (two) rhi = bc_load_block(lines, phi);    // most narrow intervals sit in one sector
+            n_sect += two ? 1u : 0u;
             const uint32_t olo = bc_block_rank1(rlo, plo, c), ohi = bc_block_rank1(rhi, phi, c);
             if (c > 3u || ohi == olo) act = false;
             else {
-                k = sel4(Cv.x, Cv.y, Cv.z, Cv.w, c) + olo + 1u; s = ohi - olo; ++t;
+                k = Ctab[(qid & 1u) * 4u + c] + olo + 1u; s = ohi - olo; ++t;
                 if (t == m) { emit = true; act = false; }
+                else c = BC_PREP_BASE(pp[t]);             // needed by the NEXT step's popc only: off the critical path
             }
         }
         if (__any_sync(0xffffffffu, emit)) {
             uint32_t kf = k;
-            if (emit && !(qid & 1u)) kf = replay_k2(lines, primary, Cv, pp, k0, s0, k2, t0, t);
+            if (emit && !(qid & 1u)) kf = replay_k2(lines, primary, sc.Cv0, pp, k0, s0, k2, t0, t);
             emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, kf, s, dz);
         }
     }
     // park: strand 0 first brings k2 up to date
     const uint32_t am = __ballot_sync(0xffffffffu, act);
     if (act) {
-        if (!(qid & 1u) && t > t0) k2 = replay_k2(lines, primary, Cv, pp, k0, s0, k2, t0, t);
-        ent_store(Cq, __popc(am & lt_mask), qid, k, s, k2, t, (dz << 8) | ((m - 1u) << 16));
+        if (!(qid & 1u) && t > t0) k2 = replay_k2(lines, primary, sc.Cv0, pp, k0, s0, k2, t0, t);
+        ent_store(Cq, __popc(am & lt_mask), qid, k, s, k2, t | (c << 27), (dz << 8) | ((m - 1u) << 16));
     }
     __syncwarp();
     return __popc(am);
@@ -246,6 +266,7 @@ __device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const S
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
+    __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
     uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
@@ -265,9 +286,12 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     sc.Cv0 = make_uint4(p.ix.bwt[1].C[0], p.ix.bwt[1].C[1], p.ix.bwt[1].C[2], p.ix.bwt[1].C[3]);
     sc.Cv1 = make_uint4(p.ix.bwt[0].C[0], p.ix.bwt[0].C[1], p.ix.bwt[0].C[2], p.ix.bwt[0].C[3]);
 
+    if (threadIdx.x < 8) Ctab[threadIdx.x] = p.ix.bwt[threadIdx.x < 4 ? 1 : 0].C[threadIdx.x & 3];
+    __syncthreads();
     uint32_t bb = 1u << 24, bcnt = 0, ccnt = 0, gsp = 0, pool_max = 0;   // ring bottom, counts, spilled blocks
     bool more = true, force_drain = false;
-    unsigned long long n_nodes = 0, n_sect = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0, n_cancel = 0, n_spill = 0;
+    // 32-bit statistics, flushed to the 64-bit global counters at every intake and at the end
+    uint32_t n_cnodes = 0, n_xsect = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0, n_cancel = 0, n_spill = 0;
 
     for (;;) {
         // ---- ring <-> global: keep the hot top of the branch stack on chip --------------------------
@@ -288,6 +312,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         }
         // ---- intake: new root states while the branch stack is shallow ------------------------
         if (more && bcnt < 32u && gsp == 0u && ccnt + 32u <= CCAP) {
+            flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+            n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             uint32_t need = 32u - bcnt;
             unsigned long long tk = 0;
             if (lane == 0) tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
@@ -295,17 +321,17 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             if (tk + need >= nq) more = false;
             unsigned long long q = tk + lane;
             bool ok = lane < need && q < nq;
-            uint32_t m = 0;
+            uint32_t m = 0, pr = 0;
             if (ok) {
                 m = p.reads.len[q >> 1];
-                uint32_t pr = p.ws.prep[(size_t)q * p.ws.stride];
+                pr = p.ws.prep[(size_t)q * p.ws.stride];
                 ok = m >= 1 && m <= p.reads.max_len && (int)BC_PREP_D(pr) <= z && (int)BC_PREP_DS(pr) <= seed_z;
             }
             uint32_t mask = __ballot_sync(0xffffffffu, ok);
             if (ok) {
                 uint32_t r = __popc(mask & lt_mask);
                 if (z > 0) ent_store(P, (bb + bcnt + r) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
-                else ent_store(Cq, ccnt + r, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
+                else ent_store(Cq, ccnt + r, (uint32_t)q, 0u, full, 0u, BC_PREP_BASE(pr) << 27, (m - 1) << 16);
             }
             if (z > 0) bcnt += __popc(mask); else ccnt += __popc(mask);
             __syncwarp();
@@ -315,9 +341,9 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 
         if (ccnt > 0 && (ccnt >= 32u || bcnt == 0 || force_drain)) {
             uint32_t nn = 0, ns_ = 0, st_ = 0;
-            ccnt = chain_phase(p, sc, Cq, ccnt, (bcnt == 0 && gsp == 0 && !more) || force_drain, ctr, nn, ns_, st_);
+            ccnt = chain_phase(p, sc, Ctab, Cq, ccnt, (bcnt == 0 && gsp == 0 && !more) || force_drain, ctr, nn, ns_, st_);
             force_drain = false;
-            n_nodes += nn; n_sect += ns_; n_csteps += st_;
+            n_cnodes += nn; n_xsect += ns_; n_csteps += st_;
             continue;
         }
 
@@ -347,16 +373,17 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         }
         const uint32_t qb = BC_PREP_BASE(pr0);
         uint32_t nk[4] = {0, 0, 0, 0}, ns[4] = {0, 0, 0, 0}, nk2[4] = {0, 0, 0, 0};
+        bool straddle = false;
         if (has_base || del_ok) {
             const uint4 *lines = strand ? sc.lines1 : sc.lines0;
             const uint32_t primary = strand ? sc.primary1 : sc.primary0;
-            const uint4 Cv = strand ? sc.Cv1 : sc.Cv0;
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             uint32_t olo[4], ohi[4];
             bc_rank4(lines, plo, olo);
             bc_rank4(lines, phi, ohi);
-            n_sect += 1u + ((plo >> 6) != (phi >> 6) ? 1u : 0u);
+            straddle = (plo >> 6) != (phi >> 6);
+            const uint4 Cv = *reinterpret_cast<const uint4 *>(Ctab + strand * 4u);
             const uint32_t Cc[4] = {Cv.x, Cv.y, Cv.z, Cv.w};
             uint32_t acc = k2 + s;                       // k2 + dollar + prefix, built below
 #pragma unroll
@@ -383,6 +410,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         const uint32_t de_lo = (uint32_t)t | (2u << 9) | ((uint32_t)d_go << 11) | ((uint32_t)d_ge << 19);
         const uint32_t de_hi = (uint32_t)(sd + in_seed_del) | ((uint32_t)nd1 << 8) | m_bits;
         const uint32_t in_lo = tn | (1u << 9) | ((uint32_t)i_go << 11) | ((uint32_t)i_ge << 19);
+        const uint32_t cb0 = qb << 27, cb1 = BC_PREP_BASE(pr1) << 27;   // first base of a chain child (bits 27-29)
         const bool last1 = nd1 == z;                     // children that cost a difference exhaust the budget
         const bool term_base = (int)tn == m;             // children that consume W[t] finish the read
         const bool term_del = t == m;
@@ -438,7 +466,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         uint32_t cpos = ccnt + (excl >> 16);
         bcnt = bcnt - akeep + (tot & 0xFFFFu);
         ccnt += tot >> 16;
-        n_nodes += akeep; n_bnodes += akeep; ++n_bsteps;
+        n_bnodes += akeep; ++n_bsteps;
+        n_xsect += (act && straddle) ? 1u : 0u;
 
         if (pbits) {
             if (pbits & 1u) {
@@ -448,19 +477,19 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 if (pbits & (2u << b)) {
-                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], ma_lo, mm_hi);
+                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], ma_lo | cb1, mm_hi);
                     else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], ma_lo, mm_hi);
                 }
             }
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 if (pbits & (32u << b)) {
-                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], de_lo, de_hi);
+                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], de_lo | cb0, de_hi);
                     else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], de_lo, de_hi);
                 }
             }
             if (pbits & 512u) {
-                if (last1) ent_store(Cq, cpos++, qid, k, s, k2, in_lo, mm_hi);
+                if (last1) ent_store(Cq, cpos++, qid, k, s, k2, in_lo | cb1, mm_hi);
                 else ent_store(P, (bpos++) & BM, qid, k, s, k2, in_lo, mm_hi);
             }
         }
@@ -479,19 +508,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         }
         __syncwarp();
     }
-    // per-warp statistics
-    for (int o = 16; o > 0; o >>= 1) n_sect += __shfl_down_sync(0xffffffffu, n_sect, o);
-    if (lane == 0) {
-        atomicAdd(&ctr[BC_CTR_NODES], n_nodes);
-        atomicAdd(&ctr[BC_CTR_LOOKUPS], 2ull * n_nodes);
-        atomicAdd(&ctr[BC_CTR_LINES], n_sect);
-        atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
-        atomicAdd(&ctr[BC_CTR_BSTEPS], n_bsteps);
-        atomicAdd(&ctr[BC_CTR_BNODES], n_bnodes);
-        atomicAdd(&ctr[BC_CTR_CSTEPS], n_csteps);
-        atomicAdd(&ctr[BC_CTR_CANCEL], n_cancel);
-        atomicAdd(&ctr[BC_CTR_SPILL], n_spill);
-    }
+    flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+    if (lane == 0) atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
 }
 
 }  // namespace
