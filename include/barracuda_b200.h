@@ -157,6 +157,14 @@ int bc_index_build_host(const uint8_t *text, uint64_t n, uint32_t occ_interval, 
                         int n_threads, bc_index_host **out);
 int bc_index_host_free(bc_index_host *h);
 
+/* Measured denominator of the metric "Occ lookups/s vs the random-sector roofline":
+ * every thread issues independent uniformly random 32-byte-aligned 256-bit loads (the access one
+ * rank query makes) over d_table; timed with CUDA events on the stream.  d_table: DEVICE, 32-byte
+ * aligned, table_bytes >= 64 (much larger than L2 => HBM rate; L2-sized => on-chip rate);
+ * d_sink: DEVICE, >= 4 bytes; sectors_per_second: HOST out.  Not part of the hot path. */
+int bc_measure_random_sectors(const void *d_table, size_t table_bytes, uint32_t loads_per_thread, void *d_sink,
+                              void *cuda_stream, double *sectors_per_second);
+
 const char *bc_strerror(int status);
 
 #ifdef __cplusplus

@@ -75,11 +75,12 @@ def lib():
         L.bc_set_geometry.argtypes = [vp, u32, u32]
         L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
+        L.bc_measure_random_sectors.argtypes = [vp, C.c_size_t, u32, vp, vp, C.POINTER(C.c_double)]
         L.bc_strerror.argtypes = [i32]
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
                   "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_index_build_host",
-                  "bc_index_host_free"):
+                  "bc_index_host_free", "bc_measure_random_sectors"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -379,3 +380,18 @@ def bc_locate(ix: DeviceIndex, rows, stream=None):
                              _stream_ptr(torch, stream))
     _check(rc, "bc_locate")
     return pos
+
+
+def bc_measure_random_sectors(table_bytes: int, loads_per_thread: int = 256, device="cuda:0", stream=None) -> float:
+    """Random 32-byte-sector load rate (sectors/s) over a torch-allocated table of `table_bytes`."""
+    torch = _torch()
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        table = torch.empty(table_bytes // 4, dtype=torch.int32, device=dev)
+        table.fill_(0x5A5A5A5A)
+        sink = torch.zeros(4, dtype=torch.int32, device=dev)
+        out = C.c_double(0.0)
+        rc = lib().bc_measure_random_sectors(C.c_void_p(table.data_ptr()), table.numel() * 4, loads_per_thread,
+                                             C.c_void_p(sink.data_ptr()), _stream_ptr(torch, stream), C.byref(out))
+    _check(rc, "bc_measure_random_sectors")
+    return float(out.value)

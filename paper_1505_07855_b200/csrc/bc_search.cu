@@ -98,7 +98,9 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 // One pool per warp holds two stacks: BRANCH states (budget left, d < z) grow up from slot 0,
 // Per warp: a RING of BRANCH states (budget left, d < z), whose cold bottom spills to global memory in
 // blocks of 32, and a stack of CHAIN states (budget exhausted, d == z: only exact matching follows).
+#ifndef BC_SEARCH_MAX_THREADS
 #define BC_SEARCH_MAX_THREADS 256
+#endif
 #ifndef BC_SEARCH_MIN_CTAS
 #define BC_SEARCH_MIN_CTAS 3
 #endif

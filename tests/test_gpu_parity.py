@@ -100,6 +100,47 @@ def test_config1_full_size():
     assert int(off[-1]) >= 0.9 * reads.n_reads
 
 
+def test_config2_full_size_in_the_bench_configuration():
+    """configs[1] of BASELINE.json at FULL size, launched as bench.py launches it (one batch of
+    200,000 reads, default geometry): reads sampled across the whole batch are compared with the
+    oracle one by one, and properties that hold at any size are checked on the full output."""
+    cfg, p = pair_for("2", sd.CONFIGS["2"].n)
+    reads = sd.make_reads(cfg, p.T)
+    opts = cfg.opts.astuple()
+    b2, nm, off, ln = sd.pack_reads(reads.codes)
+    off_g, hits_g, _ = bc.bc_align_batch_host(p.ix, bc.HostReads(b2, None, off, ln), opts)
+    st = bc.bc_last_stats(p.ix)
+    assert off_g.size == reads.n_reads + 1 and int(off_g[-1]) == hits_g.size
+    assert np.all(np.diff(off_g.astype(np.int64)) >= 0)
+    assert np.all(hits_g["k"] <= hits_g["l"]) and np.all(hits_g["l"] <= cfg.n) and np.all(hits_g["d"] <= opts[0])
+    assert np.all(hits_g["zero"] == 0) and np.all(hits_g["strand"] <= 1)
+    # sorted by (strand, k, l) and unique inside every read
+    rid = np.repeat(np.arange(reads.n_reads), np.diff(off_g.astype(np.int64)))
+    same_read = rid[1:] == rid[:-1]
+    s0, s1 = hits_g["strand"][:-1], hits_g["strand"][1:]
+    k0, k1 = hits_g["k"][:-1], hits_g["k"][1:]
+    l0, l1 = hits_g["l"][:-1], hits_g["l"][1:]
+    increasing = (s1 > s0) | ((s1 == s0) & ((k1 > k0) | ((k1 == k0) & (l1 > l0))))
+    assert np.all(increasing[same_read])                              # strictly by (strand, k, l): sorted and deduplicated
+    assert st["nodes"] > 0 and st["lookups"] == 2 * st["nodes"] and st["lines"] >= st["nodes"]
+    # sampled reads, one by one
+    rng = np.random.default_rng(2)
+    pick = np.sort(rng.choice(reads.n_reads, size=3000, replace=False))
+    off_o, hits_o = p.oracle.align(reads.codes[pick], opts)
+    for j, r in enumerate(pick.tolist()):
+        g = hits_g[int(off_g[r]):int(off_g[r + 1])]
+        o = hits_o[int(off_o[j]):int(off_o[j + 1])]
+        assert g.tobytes() == o.tobytes(), r
+    # located positions of unique hits point back at where the read was drawn from (no indel drift > 3)
+    uniq = np.nonzero(np.diff(off_g.astype(np.int64))[pick] == 1)[0][:500]
+    rows = np.asarray([hits_g[int(off_g[pick[u]])]["k"] for u in uniq], np.uint32)
+    pos = bc.bc_locate(p.ix, rows).cpu().numpy().view(np.uint32).astype(np.int64)
+    strand = np.asarray([hits_g[int(off_g[pick[u]])]["strand"] for u in uniq])
+    exp = np.where(reads.strand[pick[uniq]] == 0, reads.anchor[pick[uniq]], reads.anchor[pick[uniq]] - cfg.m)
+    ok = (np.abs(pos - exp) <= 3) & (strand == reads.strand[pick[uniq]])
+    assert ok.mean() > 0.95
+
+
 @pytest.mark.parametrize("name,n,n_reads", [("2", 2_000_000, 1500), ("3", 3_000_000, 1500), ("4", 3_000_000, 1000),
                                              ("5a", 1_000_000, 300), ("5b", 3_000_000, 1000)])
 def test_config_recipes_scaled(name, n, n_reads):
