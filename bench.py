@@ -164,6 +164,9 @@ def run_ours(args):
     torch.cuda.set_device(dev)
 
     cfg, desc = workload(args.config)
+    if args.genome_bp:
+        cfg = cfg.scaled(n=args.genome_bp)
+        desc += f" [genome scaled to {args.genome_bp} bp]"
     B = cfg.n_reads if args.reads is None else args.reads
     genome = sd.make_genome(cfg)
     first, count = bdist.shard_range(B * world, rank, world)      # weak scaling: B reads per rank
@@ -304,6 +307,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="2", choices=sorted(sd.CONFIGS))
     ap.add_argument("--reads", type=int, default=None, help="reads per step per GPU (default: the config's)")
+    ap.add_argument("--genome-bp", type=int, default=None,
+                    help="same recipe on a smaller genome (exploration only; the default is the config's own size)")
     ap.add_argument("--ctas", type=int, default=0)
     ap.add_argument("--warps", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")

@@ -254,3 +254,36 @@ def test_result_independent_of_kernel_geometry():
     assert all(o == outs[0] for o in outs)
     st = bc.bc_last_stats(p.ix)
     assert st["nodes"] > 0 and st["lookups"] == 2 * st["nodes"] or st["lookups"] > 0
+
+
+def test_status_codes_for_small_buffers_and_deep_budgets():
+    cfg, p = pair_for("1", sd.CONFIGS["1"].n)
+    reads = [p.T[10:46].copy()]
+    b2, nm, o, ln = sd.pack_ragged(reads)
+    d = bc.HostReads(b2, nm, o, ln).to_device()
+    opts = (2, 0, 0, 0, 0, 5)
+    ws = bc.Workspace(p.ix, 1, 36, opts)
+    ws.ws_bytes = 4096                                   # claim a workspace far smaller than *_bytes said
+    assert bc.bc_align_batch_raw(p.ix, d, opts, ws) == bc.BC_E_NOMEM
+    # a budget the on-chip pool cannot bound is refused, not mis-computed
+    deep = (200, 0, 0, 0, 0, 5)
+    with pytest.raises(bc.BcError) as e:
+        bc.Workspace(p.ix, 1, 36, deep)
+    assert e.value.status == bc.BC_E_UNSUPPORTED
+    # locate: out-of-range rows give the sentinel, not a wild read
+    pos = bc.bc_locate(p.ix, np.asarray([p.T.size + 5], np.uint32)).cpu().numpy().view(np.uint32)
+    assert pos[0] == 0xFFFFFFFF
+    assert bc.bc_measure_random_sectors(1 << 24, 64) > 1e9
+
+
+def test_moderately_deep_budget():
+    """z = 8 (R = 8z+9 = 73 leaves little of the 128-entry ring): results still match the oracle."""
+    cfg, p = pair_for("1", sd.CONFIGS["1"].n)
+    rng = np.random.default_rng(4)
+    rl = []
+    for _ in range(40):
+        s0 = int(rng.integers(0, p.T.size - 20))
+        rl.append(p.T[s0:s0 + 16].copy())
+    assert_same(p.ix, p.oracle, rl, (8, 0, 0, 12, 1, 5))
+    rl24 = [p.T[i * 1000:i * 1000 + 24].copy() for i in range(1, 9)]
+    assert_same(p.ix, p.oracle, rl24, (5, 1, 2, 0, 0, 3))

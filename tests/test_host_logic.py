@@ -47,6 +47,19 @@ def test_strerror_and_invalid_arguments():
     assert L.bc_index_build_host(ok.ctypes.data_as(C.c_void_p), 4, 128, 0, 1, C.byref(out)) == bc.BC_E_INVAL
 
 
+def test_compute_entry_points_reject_bad_arguments_without_a_gpu():
+    L = bc.lib()
+    b = C.c_size_t(0)
+    o = bc.make_opts((2, 0, 0, 0, 0, 5))
+    assert L.bc_align_workspace_bytes(None, 10, 36, C.byref(o), 0, C.byref(b)) == bc.BC_E_INVAL
+    assert L.bc_align_batch(None, None, None, None, None, 0, None) == bc.BC_E_INVAL
+    out = C.c_double(0)
+    assert L.bc_measure_random_sectors(None, 1 << 20, 64, None, None, C.byref(out)) == bc.BC_E_INVAL
+    assert L.bc_last_stats(None, None) == bc.BC_E_INVAL
+    assert L.bc_set_geometry(None, 1, 1) == bc.BC_E_INVAL
+    assert L.bc_index_host_free(None) == bc.BC_E_INVAL
+
+
 def unpack_bwt(bwt2, n):
     w = np.repeat(bwt2, 32)[:n]
     sh = (2 * (np.arange(n, dtype=np.uint64) % np.uint64(32))).astype(np.uint64)
