@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(256) bc_random_sector_kernel(const uint4 *tabl
 #pragma unroll
         for (int u = 0; u < 4; ++u) {                    // four independent loads in flight per thread
             h = mix64(h + u);
-            const uint4 *q = table + (h % n_sectors) * 2;
+            const uint4 *q = table + __umul64hi(h, n_sectors) * 2;   // uniform in [0, n_sectors) without a 64-bit division
             asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                          : "=r"(v[u][0]), "=r"(v[u][1]), "=r"(v[u][2]), "=r"(v[u][3]), "=r"(v[u][4]), "=r"(v[u][5]),
                            "=r"(v[u][6]), "=r"(v[u][7])

@@ -94,8 +94,7 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 // Pool entry = 24 bytes, array-of-structures, moved with three 64-bit shared-memory accesses:
 //   {qid, k} {s, k2} {mlo, mhi}
 //   mlo = t (bits 0-8) | st (9-10; 0 = M, 1 = I, 2 = D) | n_go (11-18) | n_ge (19-26)
-//   mhi = seed_d (0-7) | d (8-15) | m-1 (16-23)
-// One pool per warp holds two stacks: BRANCH states (budget left, d < z) grow up from slot 0,
+//   mhi = seed_d (0-7) | d (8-15) | m-1 (16-23);  chain entries also carry their next base in mlo bits 27-29
 // Per warp: a RING of BRANCH states (budget left, d < z), whose cold bottom spills to global memory in
 // blocks of 32, and a stack of CHAIN states (budget exhausted, d == z: only exact matching follows).
 #ifndef BC_SEARCH_MAX_THREADS
@@ -128,28 +127,6 @@ __device__ __noinline__ void emit_hits(BcRawHit *arena, unsigned long long arena
     }
 }
 
-// Strand 0 only: forward-interval start after exactly matching W[t0..t1) from the state
-// (k, s, k2) -- the bidirectional update of SURVEY C7 (R), replayed where a chain needs it.
-__device__ __noinline__ uint32_t replay_k2(const uint4 *lines, uint32_t primary, uint4 Cv, const uint16_t *pp, uint32_t k,
-                                           uint32_t s, uint32_t k2, uint32_t t0, uint32_t t1) {
-    for (uint32_t t = t0; t < t1; ++t) {
-        const uint32_t c = BC_PREP_BASE(pp[t]);
-        uint32_t olo[4], ohi[4];
-        bc_rank4(lines, k - (k > primary ? 1u : 0u), olo);
-        bc_rank4(lines, k + s - (k + s > primary ? 1u : 0u), ohi);
-        uint32_t acc = k2 + s;
-#pragma unroll
-        for (int b = 0; b < 4; ++b) acc -= ohi[b] - olo[b];           // k2 + (1 if '$' is in the interval)
-#pragma unroll
-        for (int b = 0; b < 4; ++b) if ((uint32_t)b < c) acc += ohi[b] - olo[b];
-        k2 = acc;
-        const uint32_t o = sel4(olo[0], olo[1], olo[2], olo[3], c);
-        s = sel4(ohi[0], ohi[1], ohi[2], ohi[3], c) - o;
-        k = sel4(Cv.x, Cv.y, Cv.z, Cv.w, c) + o + 1u;
-    }
-    return k2;
-}
-
 // per-warp statistics: n_xsect is per lane (second sectors of a rank pair), the rest warp-uniform
 __device__ __noinline__ void flush_stats(unsigned long long *ctr, uint32_t lane, uint32_t n_cnodes, uint32_t n_xsect,
                                          uint32_t n_bsteps, uint32_t n_bnodes, uint32_t n_csteps, uint32_t n_cancel,
@@ -172,78 +149,80 @@ __device__ __noinline__ void flush_stats(unsigned long long *ctr, uint32_t lane,
 struct SearchConsts {            // warp-uniform values the phases share; suffix = strand
     const uint4 *lines0, *lines1;   // index the strand's query is matched on (strand 0: reverse index)
     uint32_t primary0, primary1;
-    uint4 Cv0, Cv1;
 };
 
 // ---------------------------------------------------------------------------------------------
-// CHAIN phase (see the kernel's header comment).  Returns the number of parked chain states.
+// CHAIN steps (see the kernel's header comment): while the stack of strand S holds a warp's worth
+// of chain states (or, when draining, anything at all), pop 32, extend each by ONE exactly matching
+// base -- one symbol's rank at both interval ends -- and push the survivors back compacted.  Flat
+// cost per node whatever the chain lengths; lanes are full whenever 32 states are pending.
+// Strand 0 (searched on the reverse index) also advances the forward interval start k2 by the
+// bidirectional update of SURVEY C7 (R): '$' + the symbols smaller than c inside the interval.
+// Stack layout inside the chain area Cq[0..CCAP): strand 1 grows up from 0, strand 0 down from CCAP-1.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const SearchConsts &sc, const uint32_t *Ctab,
-                                                uint2 *Cq, uint32_t ccnt, bool must_finish, unsigned long long *ctr,
-                                                uint32_t &n_nodes, uint32_t &n_sect, uint32_t &n_steps) {
+template <bool S0>
+__device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4 *lines, uint32_t primary,
+                                            const uint32_t *Cs, uint2 *Cq, uint32_t CCAP, uint32_t &cnt,
+                                            bool drain, unsigned long long *ctr, uint32_t &n_nodes, uint32_t &n_xsect,
+                                            uint32_t &n_steps) {
     const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u;
-    bool act = false;
-    uint32_t qid = 0, k = 0, s = 0, k2 = 0, t = 0, m = 0, dz = 0, c = 0;
-    uint32_t k0 = 0, s0 = 0, t0 = 0;                      // strand 0: the state k2 belongs to
-    const uint16_t *pp = p.ws.prep;
-    const uint4 *lines = sc.lines0;
-    uint32_t primary = 0;
-    for (;;) {
-        const uint32_t idle = __ballot_sync(0xffffffffu, !act);
-        if (idle && ccnt) {
-            const uint32_t r = __popc(idle & lt_mask);
-            if (!act && r < ccnt) {
-                const uint2 *e = Cq + (ccnt - 1u - r) * 3u;
-                const uint2 a0 = e[0], a1 = e[1], a2 = e[2];
-                qid = a0.x; k = a0.y; s = a1.x; k2 = a1.y;
-                t = a2.x & 511u; c = a2.x >> 27;          // the entry carries the base W[t] (strand-adjusted)
-                m = ((a2.y >> 16) & 255u) + 1u; dz = (a2.y >> 8) & 255u;
-                k0 = k; s0 = s; t0 = t;
-                const uint32_t strand = qid & 1u;
-                pp = p.ws.prep + (size_t)qid * p.ws.stride;
-                lines = strand ? sc.lines1 : sc.lines0; primary = strand ? sc.primary1 : sc.primary0;
-                act = true;
-            }
-            const uint32_t take = __popc(idle);
-            ccnt -= take < ccnt ? take : ccnt;
-            __syncwarp();
-        }
-        const uint32_t am = __ballot_sync(0xffffffffu, act);
-        if (am == 0) return 0;
-        if (!must_finish && ccnt == 0 && __popc(am) < 16) break;      // park the survivors
-        n_nodes += __popc(am);
-        ++n_steps;
-        bool emit = false;
+    while (cnt >= 32u || (drain && cnt > 0u)) {
+        const uint32_t a = cnt < 32u ? cnt : 32u;
+        const bool act = lane < a;
+        uint32_t qid = 0, k = 0, s = 0, k2 = 0, mlo = 0, mhi = 0;
         if (act) {
-            const uint32_t x0 = k, x1 = k + s;
-            const uint32_t plo = x0 - (x0 > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
+            const uint2 *e = Cq + (S0 ? CCAP - cnt + lane : cnt - 1u - lane) * 3u;
+            const uint2 a0 = e[0], a1 = e[1], a2 = e[2];
+            qid = a0.x; k = a0.y; s = a1.x; k2 = a1.y; mlo = a2.x; mhi = a2.y;
+        }
+        cnt -= a;
+        __syncwarp();
+        n_nodes += a; ++n_steps;
+        uint32_t t = mlo & 511u;
+        const uint32_t c = mlo >> 27, m = ((mhi >> 16) & 255u) + 1u;
+        bool alive = false, emit = false;
+        if (act) {
+            const uint32_t x1 = k + s;
+            const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             const bool two = (plo >> 6) != (phi >> 6);
             const BcBlockRegs rlo = bc_load_block(lines, plo);
-            BcBlockRegs rhi = rlo;
-            if (two) rhi = bc_load_block(lines, phi);    // most narrow intervals sit in one sector
-            n_sect += two ? 1u : 0u;
-            const uint32_t olo = bc_block_rank1(rlo, plo, c), ohi = bc_block_rank1(rhi, phi, c);
-            if (c > 3u || ohi == olo) act = false;
-            else {
-                k = Ctab[(qid & 1u) * 4u + c] + olo + 1u; s = ohi - olo; ++t;
-                if (t == m) { emit = true; act = false; }
-                else c = BC_PREP_BASE(pp[t]);             // needed by the NEXT step's popc only: off the critical path
+            n_xsect += two ? 1u : 0u;
+            // strand 0 also needs one OTHER symbol's count for the forward start k2 (see below):
+            // x = A when c is A or C, x = T when c is G or T
+            const uint32_t x = c < 2u ? 0u : 3u;
+            uint32_t olo = bc_block_rank1(rlo, plo, c), ohi, xlo = 0, xhi = 0;
+            if (S0) xlo = bc_block_rank1(rlo, plo, x);
+            if (two) {                                    // most narrow intervals sit in one sector
+                const BcBlockRegs rhi = bc_load_block(lines, phi);
+                ohi = bc_block_rank1(rhi, phi, c);
+                if (S0) xhi = bc_block_rank1(rhi, phi, x);
+            } else {
+                ohi = bc_block_rank1(rlo, phi, c);
+                if (S0) xhi = bc_block_rank1(rlo, phi, x);
+            }
+            if (c <= 3u && ohi != olo) {
+                if (S0) {
+                    // children split the forward interval in the order $,A,C,G,T:
+                    //   A: k2 + dollar;  C: k2 + dollar + nA;  G: k2 + s - nT - nG;  T: k2 + s - nT
+                    const uint32_t dollar = s - (phi - plo), nx = xhi - xlo, nc_ = ohi - olo;
+                    k2 = c == 0u ? k2 + dollar : (c == 1u ? k2 + dollar + nx : (c == 2u ? k2 + s - nx - nc_ : k2 + s - nc_));
+                }
+                k = Cs[c] + olo + 1u; s = ohi - olo; ++t;
+                emit = t == m; alive = !emit;
             }
         }
-        if (__any_sync(0xffffffffu, emit)) {
-            uint32_t kf = k;
-            if (emit && !(qid & 1u)) kf = replay_k2(lines, primary, sc.Cv0, pp, k0, s0, k2, t0, t);
-            emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, kf, s, dz);
+        uint32_t nb = 0;
+        if (alive) nb = BC_PREP_BASE(p.ws.prep[(size_t)qid * p.ws.stride + t]);
+        const uint32_t smask = __ballot_sync(0xffffffffu, alive);
+        if (alive) {
+            const uint32_t r = __popc(smask & lt_mask);
+            ent_store(Cq, S0 ? CCAP - 1u - cnt - r : cnt + r, qid, k, s, k2, t | (nb << 27), mhi);
         }
+        cnt += __popc(smask);
+        if (__any_sync(0xffffffffu, emit))
+            emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, S0 ? k2 : k, s, (mhi >> 8) & 255u);
+        __syncwarp();
     }
-    // park: strand 0 first brings k2 up to date
-    const uint32_t am = __ballot_sync(0xffffffffu, act);
-    if (act) {
-        if (!(qid & 1u) && t > t0) k2 = replay_k2(lines, primary, sc.Cv0, pp, k0, s0, k2, t0, t);
-        ent_store(Cq, __popc(am & lt_mask), qid, k, s, k2, t | (c << 27), (dz << 8) | ((m - 1u) << 16));
-    }
-    __syncwarp();
-    return __popc(am);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -254,9 +233,9 @@ __device__ __forceinline__ uint32_t chain_phase(const BcSearchParams &p, const S
 //    surviving children, a warp scan assigns pool slots, and each lane writes its own children:
 //    those that still have budget to the branch stack (match child deepest), those with d == z to
 //    the chain stack; terminal children are emitted.
-//  * CHAIN phase: lanes pull chain states and extend them by exact matching only (one symbol's
-//    rank at both interval ends per step, no pool traffic), refilling from the chain stack as they
-//    die, until the stack is dry and fewer than half the lanes are busy; survivors are parked.
+//  * CHAIN steps: whenever a strand's chain stack holds 32 states, 32 are popped, each is extended
+//    by ONE exactly matching base (one symbol's rank at both interval ends) and the survivors are
+//    pushed back compacted -- a flat cost per node, full lanes, whatever the chain lengths.
 // New queries are drawn from a global ticket counter whenever fewer than 32 branch states are
 // pending, so lanes stay busy and converged whatever the shape of the individual search trees.
 // Pool bound: a multi-lane step keeps only the leading lanes whose children leave the
@@ -272,7 +251,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
     uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
-    uint2 *Cq = P + 3u * BCAP;                                    // chain stack: slots 0 .. ccnt-1
+    uint2 *Cq = P + 3u * BCAP;                                    // chain area: strand 1 up from 0, strand 0 down from CCAP-1
     uint2 *G = p.ws.spill + ((size_t)blockIdx.x * (blockDim.x >> 5) + warp) * ((size_t)p.ws.spill_blocks * 96u);
     const uint32_t GB = p.ws.spill_blocks;
     const uint32_t lt_mask = (1u << lane) - 1u;
@@ -285,12 +264,10 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     SearchConsts sc;
     sc.lines0 = p.ix.bwt[1].lines; sc.lines1 = p.ix.bwt[0].lines;          // strand 0 searches the reverse index
     sc.primary0 = p.ix.bwt[1].primary; sc.primary1 = p.ix.bwt[0].primary;
-    sc.Cv0 = make_uint4(p.ix.bwt[1].C[0], p.ix.bwt[1].C[1], p.ix.bwt[1].C[2], p.ix.bwt[1].C[3]);
-    sc.Cv1 = make_uint4(p.ix.bwt[0].C[0], p.ix.bwt[0].C[1], p.ix.bwt[0].C[2], p.ix.bwt[0].C[3]);
 
     if (threadIdx.x < 8) Ctab[threadIdx.x] = p.ix.bwt[threadIdx.x < 4 ? 1 : 0].C[threadIdx.x & 3];
     __syncthreads();
-    uint32_t bb = 1u << 24, bcnt = 0, ccnt = 0, gsp = 0, pool_max = 0;   // ring bottom, counts, spilled blocks
+    uint32_t bb = 1u << 24, bcnt = 0, c0 = 0, c1 = 0, gsp = 0, pool_max = 0;   // ring bottom, counts (branch, chain per strand), spilled blocks
     bool more = true, force_drain = false;
     // 32-bit statistics, flushed to the 64-bit global counters at every intake and at the end
     uint32_t n_cnodes = 0, n_xsect = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0, n_cancel = 0, n_spill = 0;
@@ -313,7 +290,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             __syncwarp();
         }
         // ---- intake: new root states while the branch stack is shallow ------------------------
-        if (more && bcnt < 32u && gsp == 0u && ccnt + 32u <= CCAP) {
+        if (more && bcnt < 32u && gsp == 0u && c0 + c1 + 32u <= CCAP) {
             flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             uint32_t need = 32u - bcnt;
@@ -329,23 +306,25 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                 pr = p.ws.prep[(size_t)q * p.ws.stride];
                 ok = m >= 1 && m <= p.reads.max_len && (int)BC_PREP_D(pr) <= z && (int)BC_PREP_DS(pr) <= seed_z;
             }
-            uint32_t mask = __ballot_sync(0xffffffffu, ok);
+            const bool odd = (q & 1ull) != 0;
+            const uint32_t mask = __ballot_sync(0xffffffffu, ok);
+            const uint32_t mask1 = __ballot_sync(0xffffffffu, ok && odd), mask0 = mask & ~mask1;
             if (ok) {
-                uint32_t r = __popc(mask & lt_mask);
-                if (z > 0) ent_store(P, (bb + bcnt + r) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
-                else ent_store(Cq, ccnt + r, (uint32_t)q, 0u, full, 0u, BC_PREP_BASE(pr) << 27, (m - 1) << 16);
+                if (z > 0) ent_store(P, (bb + bcnt + __popc(mask & lt_mask)) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
+                else ent_store(Cq, odd ? c1 + __popc(mask1 & lt_mask) : CCAP - 1u - c0 - __popc(mask0 & lt_mask), (uint32_t)q,
+                               0u, full, 0u, BC_PREP_BASE(pr) << 27, (m - 1) << 16);
             }
-            if (z > 0) bcnt += __popc(mask); else ccnt += __popc(mask);
+            if (z > 0) bcnt += __popc(mask); else { c1 += __popc(mask1); c0 += __popc(mask0); }
             __syncwarp();
         }
-        if (bcnt == 0 && ccnt == 0) { if (!more) break; continue; }
-        pool_max = bcnt + ccnt > pool_max ? bcnt + ccnt : pool_max;
+        if (bcnt == 0 && c0 + c1 == 0) { if (!more) break; continue; }
+        pool_max = bcnt + c0 + c1 > pool_max ? bcnt + c0 + c1 : pool_max;
 
-        if (ccnt > 0 && (ccnt >= 32u || bcnt == 0 || force_drain)) {
-            uint32_t nn = 0, ns_ = 0, st_ = 0;
-            ccnt = chain_phase(p, sc, Ctab, Cq, ccnt, (bcnt == 0 && gsp == 0 && !more) || force_drain, ctr, nn, ns_, st_);
+        if (c1 >= 32u || c0 >= 32u || ((bcnt == 0 || force_drain) && c0 + c1 > 0u)) {
+            const bool drain = bcnt == 0 || force_drain;
+            chain_steps<false>(p, sc.lines1, sc.primary1, Ctab + 4, Cq, CCAP, c1, drain, ctr, n_cnodes, n_xsect, n_csteps);
+            chain_steps<true>(p, sc.lines0, sc.primary0, Ctab, Cq, CCAP, c0, drain, ctr, n_cnodes, n_xsect, n_csteps);
             force_drain = false;
-            n_cnodes += nn; n_xsect += ns_; n_csteps += st_;
             continue;
         }
 
@@ -434,9 +413,10 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         const uint32_t keep_t = E == 0 ? (last1 ? 1u : 0x3FFu) : 0u;
         uint32_t pbits = vbits & (~tbits | keep_t);
         uint32_t cbits = last1 ? (pbits & 0x3FEu) : 0u;
+        const uint32_t cshift = strand ? 10u : 20u;      // packed counters: branch (bits 0-9) | chain strand 1 (10-19) | strand 0 (20-29)
 
         // slots: warp scan of (branch pushes | chain pushes << 16); net growth decides who is kept
-        const uint32_t mine = (uint32_t)__popc(pbits & ~cbits) | ((uint32_t)__popc(cbits) << 16);
+        const uint32_t mine = (uint32_t)__popc(pbits & ~cbits) | ((uint32_t)__popc(cbits) << cshift);
         uint32_t incl = mine;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -444,8 +424,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             if ((int)lane >= o) incl += v;
         }
         // lanes 0..lane kept, the lanes behind un-popped: ring and chain occupancy after the step
-        const uint32_t ring_if = bcnt - (lane + 1u) + (incl & 0xFFFFu);
-        const uint32_t chain_if = ccnt + (incl >> 16);
+        const uint32_t ring_if = bcnt - (lane + 1u) + (incl & 1023u);
+        const uint32_t chain_if = c0 + c1 + ((incl >> 10) & 1023u) + (incl >> 20);
         const bool fits = act && ring_if + R <= BCAP && chain_if <= CCAP;
         uint32_t keepmask = __ballot_sync(0xffffffffu, fits);
         uint32_t akeep = keepmask == 0xffffffffu ? 32u : (uint32_t)(__ffs(~keepmask) - 1);   // leading run
@@ -455,7 +435,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             if (r0 <= BCAP && c0 <= CCAP) akeep = 1;
         }
         if (akeep == 0) {
-            if (ccnt == 0) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // cannot happen (pool bound)
+            if (c0 + c1 == 0) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // cannot happen (pool bound)
             force_drain = true;                           // nothing popped; make room first
             n_cancel += a;
             continue;
@@ -464,10 +444,12 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         n_cancel += a - akeep;
         const uint32_t tot = __shfl_sync(0xffffffffu, incl, akeep - 1u);
         const uint32_t excl = incl - mine;
-        uint32_t bpos = bb + bcnt - akeep + (excl & 0xFFFFu);         // ring index (masked at the store)
-        uint32_t cpos = ccnt + (excl >> 16);
-        bcnt = bcnt - akeep + (tot & 0xFFFFu);
-        ccnt += tot >> 16;
+        uint32_t bpos = bb + bcnt - akeep + (excl & 1023u);           // ring index (masked at the store)
+        uint32_t cpos = strand ? c1 + ((excl >> 10) & 1023u) : CCAP - 1u - c0 - (excl >> 20);
+        const uint32_t cstep = strand ? 1u : 0xFFFFFFFFu;             // strand 1 grows up, strand 0 down
+        bcnt = bcnt - akeep + (tot & 1023u);
+        c1 += (tot >> 10) & 1023u;
+        c0 += tot >> 20;
         n_bnodes += akeep; ++n_bsteps;
         n_xsect += (act && straddle) ? 1u : 0u;
 
@@ -479,19 +461,19 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 if (pbits & (2u << b)) {
-                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], ma_lo | cb1, mm_hi);
+                    if (last1) { ent_store(Cq, cpos, qid, nk[b], ns[b], nk2[b], ma_lo | cb1, mm_hi); cpos += cstep; }
                     else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], ma_lo, mm_hi);
                 }
             }
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 if (pbits & (32u << b)) {
-                    if (last1) ent_store(Cq, cpos++, qid, nk[b], ns[b], nk2[b], de_lo | cb0, de_hi);
+                    if (last1) { ent_store(Cq, cpos, qid, nk[b], ns[b], nk2[b], de_lo | cb0, de_hi); cpos += cstep; }
                     else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], de_lo, de_hi);
                 }
             }
             if (pbits & 512u) {
-                if (last1) ent_store(Cq, cpos++, qid, k, s, k2, in_lo | cb1, mm_hi);
+                if (last1) { ent_store(Cq, cpos, qid, k, s, k2, in_lo | cb1, mm_hi); cpos += cstep; }
                 else ent_store(P, (bpos++) & BM, qid, k, s, k2, in_lo, mm_hi);
             }
         }
