@@ -197,6 +197,12 @@ __global__ void write_hits(BcWorkspace ws, bc_result res, uint32_t n_reads) {
 
 }  // namespace
 
+// exclusive scan of n uint32 counts into uint64 offsets (out[n] = total); blk: n/2048 + 2 uint64 of scratch
+cudaError_t bc_exclusive_scan(const uint32_t *in, uint64_t n, uint64_t *blk, uint64_t *out, uint64_t *total_out,
+                              cudaStream_t st) {
+    return exclusive_scan(in, n, blk, out, total_out, st);
+}
+
 cudaError_t bc_launch_post(const BcSearchParams &p, bc_result res, cudaStream_t st) {
     const BcWorkspace &ws = p.ws;
     if (ws.nq == 0) return cudaSuccess;

@@ -65,6 +65,8 @@ cudaError_t bc_launch_prepare(const BcSearchParams &p, cudaStream_t st);
 cudaError_t bc_launch_search(const BcSearchParams &p, int sm_count, uint32_t ctas_per_sm, uint32_t warps_per_cta,
                              cudaStream_t st);
 cudaError_t bc_launch_post(const BcSearchParams &p, bc_result res, cudaStream_t st);
+cudaError_t bc_exclusive_scan(const uint32_t *in, uint64_t n, uint64_t *blk, uint64_t *out, uint64_t *total_out,
+                              cudaStream_t st);
 // smem bytes one pool entry takes; used by the host to size pools
 #define BC_POOL_ENTRY_BYTES 24u
 #define BC_SPILL_BLOCKS 128u          // per warp: 128 x 32 entries x 24 B = 96 KB of workspace
