@@ -132,6 +132,19 @@ int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t max_
 int bc_align_batch(const bc_index *ix, const bc_reads *reads, const bc_opts *o, bc_result *res,
                    void *d_workspace, size_t ws_bytes, void *cuda_stream);
 
+/* Best-stratum mode (the early-terminating behaviour of production short-read
+ * aligners, "85 % match uniquely"): per read, exactly the hits of bc_align_batch whose
+ * d <= min(d_min + stratum_plus, z), d_min = the read's smallest d over both strands; reads without
+ * a hit within z stay empty.  Computed by iterative deepening over the budget with bc_align_batch
+ * as the inner step, so well-matching reads never pay for the deep budgets.  Same buffers, layout,
+ * ordering and status codes as bc_align_batch (n_hits_needed on BC_E_OVERFLOW refers to the pass
+ * that failed); bc_last_stats afterwards holds the sums over the passes and [15] = passes run.
+ * hits_capacity in the *_bytes call must be the capacity later passed in bc_result. */
+int bc_align_best_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t max_len, const bc_opts *o,
+                                  uint32_t raw_hits_per_read, uint64_t hits_capacity, size_t *bytes);
+int bc_align_batch_best(const bc_index *ix, const bc_reads *reads, const bc_opts *o, int32_t stratum_plus,
+                        bc_result *res, void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
 /* SA-interval row -> text coordinate: pos[i] = SA_fwd[rows[i]] by LF-walk to
  * a sampled row.  d_rows, d_pos: DEVICE.  rows[i] must be in [0, n]. */
 int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream);

@@ -70,6 +70,9 @@ def lib():
         L.bc_index_free.argtypes = [vp]
         L.bc_align_workspace_bytes.argtypes = [vp, u32, u32, C.POINTER(bc_opts), u32, C.POINTER(C.c_size_t)]
         L.bc_align_batch.argtypes = [vp, C.POINTER(bc_reads), C.POINTER(bc_opts), C.POINTER(bc_result), vp, C.c_size_t, vp]
+        L.bc_align_best_workspace_bytes.argtypes = [vp, u32, u32, C.POINTER(bc_opts), u32, u64, C.POINTER(C.c_size_t)]
+        L.bc_align_batch_best.argtypes = [vp, C.POINTER(bc_reads), C.POINTER(bc_opts), C.c_int32, C.POINTER(bc_result), vp,
+                                          C.c_size_t, vp]
         L.bc_locate.argtypes = [vp, vp, u64, vp, vp]
         L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 16)]
         L.bc_set_geometry.argtypes = [vp, u32, u32]
@@ -80,7 +83,8 @@ def lib():
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
                   "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_index_build_host",
-                  "bc_index_host_free", "bc_measure_random_sectors"):
+                  "bc_index_host_free", "bc_measure_random_sectors", "bc_align_best_workspace_bytes",
+                  "bc_align_batch_best"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -395,3 +399,57 @@ def bc_measure_random_sectors(table_bytes: int, loads_per_thread: int = 256, dev
                                              C.c_void_p(sink.data_ptr()), _stream_ptr(torch, stream), C.byref(out))
     _check(rc, "bc_measure_random_sectors")
     return float(out.value)
+
+
+class BestWorkspace:
+    """Caller-owned device buffers of bc_align_batch_best."""
+
+    def __init__(self, ix: DeviceIndex, n_reads: int, max_len: int, opts, raw_hits_per_read: int = 16,
+                 hits_capacity: int | None = None):
+        torch = _torch()
+        self.ix, self.n_reads, self.max_len = ix, n_reads, max_len
+        self.opts = make_opts(opts)
+        self.raw_hits_per_read = raw_hits_per_read
+        self.hits_capacity = int(hits_capacity if hits_capacity is not None else max(1024, 4 * n_reads))
+        b = C.c_size_t(0)
+        _check(lib().bc_align_best_workspace_bytes(ix.handle, n_reads, max_len, C.byref(self.opts), raw_hits_per_read,
+                                                   self.hits_capacity, C.byref(b)), "bc_align_best_workspace_bytes")
+        self.ws_bytes = int(b.value)
+        with torch.cuda.device(ix.device):
+            self.mem = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=ix.device)
+            self.hit_offsets = torch.empty(n_reads + 1, dtype=torch.int64, device=ix.device)
+            self.hits = torch.empty(self.hits_capacity * 12, dtype=torch.uint8, device=ix.device)
+            self.needed = torch.zeros(2, dtype=torch.int64, device=ix.device)
+
+    @property
+    def ptr(self) -> int:
+        return (self.mem.data_ptr() + 255) & ~255
+
+
+def bc_align_batch_best_raw(ix: DeviceIndex, reads: DeviceReads, opts, stratum_plus: int, ws: BestWorkspace, stream=None) -> int:
+    torch = _torch()
+    o = make_opts(opts)
+    r = reads.struct()
+    res = bc_result(ws.hit_offsets.data_ptr(), ws.hits.data_ptr(), ws.hits_capacity, ws.needed.data_ptr())
+    with torch.cuda.device(ix.device):
+        return lib().bc_align_batch_best(ix.handle, C.byref(r), C.byref(o), stratum_plus, C.byref(res), C.c_void_p(ws.ptr),
+                                         ws.ws_bytes, _stream_ptr(torch, stream))
+
+
+def bc_align_batch_best(ix: DeviceIndex, reads: DeviceReads, opts, stratum_plus: int = 1, ws: BestWorkspace | None = None,
+                        stream=None):
+    """Best-stratum mode: per read the hits with d <= min(d_min + stratum_plus, z).  Grows the
+    caller-owned buffers and repeats on BC_E_OVERFLOW.  Returns (AlignResult, BestWorkspace)."""
+    if ws is None:
+        ws = BestWorkspace(ix, reads.n_reads, max(1, reads.max_len), opts)
+    for _ in range(5):
+        rc = bc_align_batch_best_raw(ix, reads, opts, stratum_plus, ws, stream)
+        need = ws.needed.cpu().numpy().view(np.uint64)
+        if rc == BC_OK:
+            return AlignResult(ws.hit_offsets, ws.hits, int(need[0]), int(need[1])), ws
+        if rc != BC_E_OVERFLOW:
+            raise BcError(rc, "bc_align_batch_best")
+        per_read = max(2 * ws.raw_hits_per_read, -(-int(need[1]) // max(1, reads.n_reads)) + 1)
+        cap = max(2 * ws.hits_capacity, int(need[0]) + 1)
+        ws = BestWorkspace(ix, reads.n_reads, max(1, reads.max_len), opts, per_read, cap)
+    raise BcError(BC_E_OVERFLOW, "bc_align_batch_best (after growing)")
