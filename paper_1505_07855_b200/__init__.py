@@ -224,7 +224,7 @@ def bc_set_geometry(ix: DeviceIndex, ctas_per_sm: int = 0, warps_per_cta: int = 
 
 
 STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry",
-              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes", "cancelled", "spill_blocks")
+              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes", "cancelled", "spill_blocks", "reserved14", "passes")
 
 
 def bc_last_stats(ix: DeviceIndex) -> dict:
