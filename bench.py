@@ -292,6 +292,24 @@ def run_ours(args):
                                 "peak_index_sized_table": rs_res / 1e9, "peak_8GiB_table_hbm": rs_hbm / 1e9,
                                 "frac_of_index_sized_peak": sect_s / rs_res, "frac_of_hbm_random_peak": sect_s / rs_hbm,
                                 "how": "bc_measure_random_sectors: 64 warps/SM, 4 independent 256-bit loads in flight per thread"}
+    # ---- optional: the step after the path -- pairing the ends, timed end to end ----
+    pair_res = None
+    if args.pair and cfg.paired:
+        lo, hi = int(cfg.frag_mu - 4 * cfg.frag_sd), int(cfg.frag_mu + 4 * cfg.frag_sd)
+        resd = bc.AlignResult(ws.hit_offsets, ws.hits, n_hits, 0)
+        one_step()                                                # the device result of the last mode run
+        pair_res = bc.bc_pair_batch(ix, resd, dreads, lo, hi, 32)   # sizes the buffers
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            pair_res = bc.bc_pair_batch(ix, resd, dreads, lo, hi, 32)
+        torch.cuda.synchronize()
+        dtp = (time.perf_counter() - t0) / args.steps
+        out["pairing"] = {"pairs_of_reads_per_s": (count // 2) / dtp, "ms_per_batch": dtp * 1e3, "window": [lo, hi],
+                          "max_occ": 32, **pair_res[2],
+                          "fragments_paired_frac": float((np.diff(pair_res[0].astype(np.int64)) > 0).mean()),
+                          "note": "bc_pair_batch on the device CSR of the step above; wall clock incl. buffer allocation "
+                                  "and the copy of the pairs to the host"}
     # ---- cpu baseline: the oracle on a bounded sample of the same batch, + parity on that sample ----
     if not args.no_cpu:
         orc, sample = calibrate_sample(cfg, genome, 12.0, count)
@@ -315,6 +333,14 @@ def run_ours(args):
         same = bool(np.array_equal(off_h[: sample + 1], off_o) and
                     hits_h[: int(off_o[-1])].tobytes() == hits_o.tobytes())
         out["parity"] = {"reads_checked": sample, "identical_to_oracle": same}
+        if pair_res is not None:                                  # brute-force pairing of the oracle's own located hits
+            from oracle.pairing import pair_reads
+            ns = sample & ~1
+            SA = orc.index(0)[0]
+            po_o, pairs_o, _ = pair_reads(SA, off_o[: ns + 1], hits_o, ln[:ns], lo, hi, 32)
+            po_g, pairs_g = pair_res[0], pair_res[1]
+            out["pairing"]["parity"] = {"pairs_of_reads_checked": ns // 2, "identical_to_oracle": bool(
+                np.array_equal(po_g[: ns // 2 + 1], po_o) and pairs_g[: int(po_o[-1])].tobytes() == pairs_o.tobytes())}
     print(json.dumps(out), flush=True)
     bdist.finish()
     return 0
@@ -334,6 +360,7 @@ def main():
     ap.add_argument("--warps", type=int, default=0)
     ap.add_argument("--best", type=int, default=None, metavar="PLUS",
                     help="best-stratum mode: keep hits with d <= min(d_min + PLUS, z) (bc_align_batch_best)")
+    ap.add_argument("--pair", action="store_true", help="also time bc_pair_batch on the result (paired configs)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-probe", action="store_true", help="skip the random-sector microbenchmark")
     args = ap.parse_args()

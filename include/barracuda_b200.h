@@ -145,6 +145,23 @@ int bc_align_best_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t
 int bc_align_batch_best(const bc_index *ix, const bc_reads *reads, const bc_opts *o, int32_t stratum_plus,
                         bc_result *res, void *d_workspace, size_t ws_bytes, void *cuda_stream);
 
+/* Pairing of the two ends of a fragment by plausible distance (SURVEY 8f NEXT-1; PAPER.md:37, :39,
+ * :104: the `sampe` step).  Input: the DEVICE CSR result of bc_align_batch / bc_align_batch_best for
+ * a batch whose reads 2i, 2i+1 are the ends of pair i, and the reads' len[] (DEVICE).  Every hit with
+ * <= max_occ occurrences is located into placements (pos, strand, d); a proper pair = one end on
+ * strand 0 at pf, the other on strand 1 at pr >= pf, pr + len(reverse end) - pf in [min_frag, max_frag].
+ * Output (DEVICE, caller-owned): per pair the records sorted by (pos1, pos2, strand1), one per key
+ * with the smallest d1+d2 (then d1); pos1/d1/strand1 belong to read 2i, pos2/d2 to read 2i+1.
+ * n_needed[4] (DEVICE): pairs after dedup, candidate pairs, placements, hits skipped for max_occ --
+ * on BC_E_OVERFLOW they say what max_placements / max_raw_pairs / pairs_capacity must be. */
+typedef struct { uint32_t min_frag, max_frag, max_occ; } bc_pair_opts;
+typedef struct { uint32_t pos1, pos2, frag; uint8_t d1, d2, strand1, zero; } bc_pair;   /* 16 bytes */
+typedef struct { uint64_t *pair_offsets; bc_pair *pairs; uint64_t pairs_capacity; uint64_t *n_needed; } bc_pair_result;
+int bc_pair_workspace_bytes(uint32_t n_reads, uint64_t max_placements, uint64_t max_raw_pairs, size_t *bytes);
+int bc_pair_batch(const bc_index *ix, const uint64_t *d_hit_offsets, const bc_hit *d_hits, const uint16_t *d_len,
+                  uint32_t n_reads, const bc_pair_opts *o, uint64_t max_placements, uint64_t max_raw_pairs,
+                  bc_pair_result *res, void *d_workspace, size_t ws_bytes, void *cuda_stream);
+
 /* SA-interval row -> text coordinate: pos[i] = SA_fwd[rows[i]] by LF-walk to
  * a sampled row.  d_rows, d_pos: DEVICE.  rows[i] must be in [0, n]. */
 int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream);

@@ -47,6 +47,19 @@ class bc_result(C.Structure):
                 ("n_hits_needed", C.c_void_p)]
 
 
+class bc_pair_opts(C.Structure):
+    _fields_ = [("min_frag", C.c_uint32), ("max_frag", C.c_uint32), ("max_occ", C.c_uint32)]
+
+
+class bc_pair_result(C.Structure):
+    _fields_ = [("pair_offsets", C.c_void_p), ("pairs", C.c_void_p), ("pairs_capacity", C.c_uint64),
+                ("n_needed", C.c_void_p)]
+
+
+PAIR_DTYPE = np.dtype([("pos1", "<u4"), ("pos2", "<u4"), ("frag", "<u4"), ("d1", "u1"), ("d2", "u1"), ("strand1", "u1"),
+                       ("zero", "u1")])
+
+
 class BcError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
@@ -73,6 +86,9 @@ def lib():
         L.bc_align_best_workspace_bytes.argtypes = [vp, u32, u32, C.POINTER(bc_opts), u32, u64, C.POINTER(C.c_size_t)]
         L.bc_align_batch_best.argtypes = [vp, C.POINTER(bc_reads), C.POINTER(bc_opts), C.c_int32, C.POINTER(bc_result), vp,
                                           C.c_size_t, vp]
+        L.bc_pair_workspace_bytes.argtypes = [u32, u64, u64, C.POINTER(C.c_size_t)]
+        L.bc_pair_batch.argtypes = [vp, vp, vp, vp, u32, C.POINTER(bc_pair_opts), u64, u64, C.POINTER(bc_pair_result), vp,
+                                    C.c_size_t, vp]
         L.bc_locate.argtypes = [vp, vp, u64, vp, vp]
         L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 16)]
         L.bc_set_geometry.argtypes = [vp, u32, u32]
@@ -84,7 +100,7 @@ def lib():
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
                   "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_index_build_host",
                   "bc_index_host_free", "bc_measure_random_sectors", "bc_align_best_workspace_bytes",
-                  "bc_align_batch_best"):
+                  "bc_align_batch_best", "bc_pair_workspace_bytes", "bc_pair_batch"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -453,3 +469,36 @@ def bc_align_batch_best(ix: DeviceIndex, reads: DeviceReads, opts, stratum_plus:
         cap = max(2 * ws.hits_capacity, int(need[0]) + 1)
         ws = BestWorkspace(ix, reads.n_reads, max(1, reads.max_len), opts, per_read, cap)
     raise BcError(BC_E_OVERFLOW, "bc_align_batch_best (after growing)")
+
+
+def bc_pair_batch(ix: DeviceIndex, result: AlignResult, reads: DeviceReads, min_frag: int, max_frag: int, max_occ: int = 32,
+                  stream=None):
+    """Pair the two ends of every fragment (reads 2i, 2i+1) by plausible distance.
+    Returns (pair_offsets uint64[n_pairs+1], pairs PAIR_DTYPE[], needed dict) on the host; buffers are
+    grown and the call repeated on BC_E_OVERFLOW."""
+    torch = _torch()
+    n_reads = reads.n_reads
+    o = bc_pair_opts(min_frag, max_frag, max_occ)
+    max_place, max_raw, cap = max(1024, 4 * n_reads), max(1024, 2 * n_reads), max(1024, n_reads)
+    for _ in range(4):
+        b = C.c_size_t(0)
+        _check(lib().bc_pair_workspace_bytes(n_reads, max_place, max_raw, C.byref(b)), "bc_pair_workspace_bytes")
+        with torch.cuda.device(ix.device):
+            mem = torch.empty(int(b.value) + 256, dtype=torch.uint8, device=ix.device)
+            poff = torch.empty(n_reads // 2 + 1, dtype=torch.int64, device=ix.device)
+            pairs = torch.empty(cap * 16, dtype=torch.uint8, device=ix.device)
+            need = torch.zeros(4, dtype=torch.int64, device=ix.device)
+            res = bc_pair_result(poff.data_ptr(), pairs.data_ptr(), cap, need.data_ptr())
+            rc = lib().bc_pair_batch(ix.handle, C.c_void_p(result.hit_offsets.data_ptr()), C.c_void_p(result.hits.data_ptr()),
+                                     C.c_void_p(reads.len.data_ptr()), n_reads, C.byref(o), max_place, max_raw, C.byref(res),
+                                     C.c_void_p((mem.data_ptr() + 255) & ~255), int(b.value), _stream_ptr(torch, stream))
+        nd = need.cpu().numpy().view(np.uint64)
+        info = {"pairs": int(nd[0]), "raw_pairs": int(nd[1]), "placements": int(nd[2]), "skipped_hits": int(nd[3])}
+        if rc == BC_OK:
+            return poff.cpu().numpy().view(np.uint64), pairs[: info["pairs"] * 16].cpu().numpy().view(PAIR_DTYPE), info
+        if rc != BC_E_OVERFLOW:
+            raise BcError(rc, "bc_pair_batch")
+        max_place = max(max_place, info["placements"] + 1)
+        max_raw = max(max_raw, info["raw_pairs"] + 1)
+        cap = max(cap, info["pairs"] + 1, info["raw_pairs"] + 1)
+    raise BcError(BC_E_OVERFLOW, "bc_pair_batch (after growing)")
