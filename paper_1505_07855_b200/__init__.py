@@ -164,9 +164,36 @@ class HostIndex:
         cnt = self.n // s.sa_interval + 1
         return np.ctypeslib.as_array(C.cast(s.sa, C.POINTER(C.c_uint32)), shape=(cnt,)), int(s.sa_interval)
 
+    def save(self, path: str):
+        """Cache the transport arrays on disk (config 5: "index built once on the host and cached")."""
+        st = self.struct
+        d = {"n": np.uint64(self.n), "sa_interval": np.uint32(st.sa_interval), "sa": self.sa_samples()[0]}
+        for name, which in (("fwd", 0), ("rev", 1)):
+            bwt2, occ, Cc, primary, oi = self.arrays(which)
+            d[name + "_bwt2"], d[name + "_occ"] = bwt2, occ
+            d[name + "_C"], d[name + "_primary"], d[name + "_oi"] = np.asarray(Cc, np.uint64), np.uint64(primary), np.uint32(oi)
+        np.savez(path, **d)
+
+    @staticmethod
+    def load(path: str) -> "HostIndex":
+        """A bc_index_host over numpy arrays read back from save(); Python owns the memory."""
+        z = np.load(path)
+        keep = {k: np.ascontiguousarray(z[k]) for k in z.files}
+        h = bc_index_host()
+        for name, b in (("fwd", h.fwd), ("rev", h.rev)):
+            b.n = int(keep["n"]); b.primary = int(keep[name + "_primary"]); b.occ_interval = int(keep[name + "_oi"])
+            b.bwt2 = keep[name + "_bwt2"].ctypes.data; b.occ = keep[name + "_occ"].ctypes.data
+            for c in range(5):
+                b.C[c] = int(keep[name + "_C"][c])
+        h.sa_interval = int(keep["sa_interval"]); h.sa = keep["sa"].ctypes.data
+        obj = HostIndex(C.pointer(h))
+        obj._owned, obj._keep = False, (keep, h)
+        return obj
+
     def free(self):
         if self._p is not None:
-            lib().bc_index_host_free(self._p)
+            if getattr(self, "_owned", True):
+                lib().bc_index_host_free(self._p)
             self._p = None
 
     def __del__(self):

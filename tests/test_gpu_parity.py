@@ -287,3 +287,18 @@ def test_moderately_deep_budget():
     assert_same(p.ix, p.oracle, rl, (8, 0, 0, 12, 1, 5))
     rl24 = [p.T[i * 1000:i * 1000 + 24].copy() for i in range(1, 9)]
     assert_same(p.ix, p.oracle, rl24, (5, 1, 2, 0, 0, 3))
+
+
+def test_autotune_keeps_parity_as_a_hard_constraint():
+    from paper_1505_07855_b200.autotune import autotune_geometry
+    cfg, p = pair_for("2", 2_000_000)
+    reads = sd.make_reads(cfg.scaled(n_reads=4000), p.T, 0, 4000)
+    opts = cfg.opts.astuple()
+    b2, nm, off, ln = sd.pack_reads(reads.codes)
+    d = bc.HostReads(b2, nm, off, ln).to_device()
+    best, table = autotune_geometry(p.ix, d, opts, candidates=((0, 0), (2, 8), (4, 6), (6, 4)), repeats=1)
+    assert all(r["identical"] for r in table if r["status"] == "ok") and best["geometry"] in [r["geometry"] for r in table]
+    off_g, hits_g = gpu_align(p.ix, list(reads.codes), opts)          # runs with the winner left set
+    off_o, hits_o = p.oracle.align(reads.codes, opts)
+    bc.bc_set_geometry(p.ix, 0, 0)
+    assert np.array_equal(off_g, off_o) and hits_g.tobytes() == hits_o.tobytes()
