@@ -70,9 +70,8 @@ __device__ __forceinline__ BcBlockRegs bc_load_block(const uint4 *lines, uint32_
     return r;
 }
 
-// all four O(., .) before position p of the '$'-less string: out[c] = #{j < p : B'[j] = c}
-__device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_t out[4]) {
-    const BcBlockRegs r = bc_load_block(lines, p);
+// all four counts from a loaded block: out[c] = #{j < p : B'[j] = c}
+__device__ __forceinline__ void bc_block_rank4(const BcBlockRegs &r, uint32_t p, uint32_t out[4]) {
     const uint32_t b = p & 63u;
     const uint64_t m = (1ull << b) - 1ull;
     const uint64_t lo = r.lo & m, hi = r.hi & m;
@@ -81,6 +80,11 @@ __device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_
     out[1] = r.c1 + nc;
     out[2] = r.c2 + ng;
     out[3] = r.c3 + nt;
+}
+
+// all four O(., .) before position p of the '$'-less string
+__device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_t out[4]) {
+    bc_block_rank4(bc_load_block(lines, p), p, out);
 }
 
 // one symbol's count from a loaded block: #{j < p : B'[j] = c}  (c > 3 gives a don't-care value)
