@@ -187,6 +187,15 @@ int bc_index_build_host(const uint8_t *text, uint64_t n, uint32_t occ_interval, 
                         int n_threads, bc_index_host **out);
 int bc_index_host_free(bc_index_host *h);
 
+/* The same construction on the GPU: suffix arrays of T$ and reverse(T)$ by prefix
+ * doubling with library radix sorts, then BWT, Occ checkpoints and SA sample in kernels.  Returns
+ * transport arrays bit-identical to bc_index_build_host's (released with bc_index_host_free).
+ * text: HOST, n codes 0..3; d_scratch: DEVICE, 256-byte aligned, >= bc_index_build_gpu_bytes
+ * (about 34 bytes per base). */
+int bc_index_build_gpu_bytes(uint64_t n, uint32_t occ_interval, uint32_t sa_interval, size_t *bytes);
+int bc_index_build_gpu(const uint8_t *text, uint64_t n, uint32_t occ_interval, uint32_t sa_interval, void *d_scratch,
+                       size_t scratch_bytes, void *cuda_stream, bc_index_host **out);
+
 /* Measured denominator of the metric "Occ lookups/s vs the random-sector roofline":
  * every thread issues independent uniformly random 32-byte-aligned 256-bit loads (the access one
  * rank query makes) over d_table; timed with CUDA events on the stream.  d_table: DEVICE, 32-byte

@@ -94,13 +94,15 @@ def lib():
         L.bc_set_geometry.argtypes = [vp, u32, u32]
         L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
+        L.bc_index_build_gpu_bytes.argtypes = [u64, u32, u32, C.POINTER(C.c_size_t)]
+        L.bc_index_build_gpu.argtypes = [vp, u64, u32, u32, vp, C.c_size_t, vp, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_measure_random_sectors.argtypes = [vp, C.c_size_t, u32, vp, vp, C.POINTER(C.c_double)]
         L.bc_strerror.argtypes = [i32]
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
                   "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_index_build_host",
                   "bc_index_host_free", "bc_measure_random_sectors", "bc_align_best_workspace_bytes",
-                  "bc_align_batch_best", "bc_pair_workspace_bytes", "bc_pair_batch"):
+                  "bc_align_batch_best", "bc_pair_workspace_bytes", "bc_pair_batch", "bc_index_build_gpu_bytes", "bc_index_build_gpu"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -529,3 +531,21 @@ def bc_pair_batch(ix: DeviceIndex, result: AlignResult, reads: DeviceReads, min_
         max_raw = max(max_raw, info["raw_pairs"] + 1)
         cap = max(cap, info["pairs"] + 1, info["raw_pairs"] + 1)
     raise BcError(BC_E_OVERFLOW, "bc_pair_batch (after growing)")
+
+
+def bc_index_build_gpu(text: np.ndarray, occ_interval: int = 128, sa_interval: int = 32, device="cuda:0",
+                       stream=None) -> HostIndex:
+    """Index construction on the GPU (prefix doubling); same transport arrays as bc_index_build_host."""
+    torch = _torch()
+    text = np.ascontiguousarray(text, dtype=np.uint8)
+    b = C.c_size_t(0)
+    _check(lib().bc_index_build_gpu_bytes(text.size, occ_interval, sa_interval, C.byref(b)), "bc_index_build_gpu_bytes")
+    dev = torch.device(device)
+    out = C.POINTER(bc_index_host)()
+    with torch.cuda.device(dev):
+        mem = torch.empty(int(b.value) + 256, dtype=torch.uint8, device=dev)
+        rc = lib().bc_index_build_gpu(text.ctypes.data_as(C.c_void_p), text.size, occ_interval, sa_interval,
+                                      C.c_void_p((mem.data_ptr() + 255) & ~255), int(b.value), _stream_ptr(torch, stream),
+                                      C.byref(out))
+    _check(rc, "bc_index_build_gpu")
+    return HostIndex(out)

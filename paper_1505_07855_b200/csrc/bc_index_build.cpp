@@ -3,7 +3,7 @@
 // role is played, for synthetic genomes, by a bucketed suffix sort: suffixes are grouped by their
 // first 12 bases (counting sort) and every bucket is then comparison-sorted on the text with an
 // 8-bytes-at-a-time comparator.  Product code: shares nothing with oracle/.
-#include "../../include/barracuda_b200.h"
+#include "bc_host_index.h"
 
 #include <algorithm>
 #include <atomic>
@@ -18,16 +18,8 @@ namespace {
 constexpr int KPFX = 12;                       // bases in the bucket key (24 bits)
 constexpr uint32_t NBUCKET = 1u << (2 * KPFX);
 
-struct BwtArrays {
-    std::vector<uint64_t> bwt2;
-    std::vector<uint32_t> occ;
-};
-
-struct HostIndexOwner {
-    bc_index_host pub;                          // must be first: the public pointer is this object
-    BwtArrays fwd, rev;
-    std::vector<uint32_t> sa;
-};
+using BwtArrays = BcBwtArrays;
+using HostIndexOwner = BcHostIndexOwner;
 
 // lexicographic compare of suffixes a,b of text[0..n) ('$' = end of text is smallest)
 struct SuffixCmp {
