@@ -83,3 +83,24 @@ def test_best_stratum_edge_cases():
     d = bc.HostReads(b2, nm, off, ln).to_device()
     ws = bc.BestWorkspace(p.ix, 2000, 51, opts, hits_capacity=100)
     assert bc.bc_align_batch_best_raw(p.ix, d, opts, 1, ws) == bc.BC_E_OVERFLOW
+
+
+def test_best_stratum_and_pairing_with_ragged_lengths_and_N():
+    """reads of different lengths (some with N) through the sub-batch gather of the best-stratum
+    mode, then through the pairing step (which uses each read's own length)."""
+    from oracle.pairing import pair_reads
+    cfg, p = pair_for("3", 3_000_000)
+    reads = sd.make_reads(cfg.scaled(n_reads=800), p.T, 0, 800)
+    rng = np.random.default_rng(8)
+    rl = [r[: int(rng.integers(40, reads.m + 1))].copy() for r in reads.codes]
+    opts = (3, 1, 2, 24, 1, 5)
+    b2, nm, off, ln = sd.pack_ragged(rl)
+    d = bc.HostReads(b2, nm, off, ln).to_device()
+    res, _ = bc.bc_align_batch_best(p.ix, d, opts, 1)
+    off_g, hits_g = res.to_numpy()
+    off_o, hits_o = p.oracle.align(rl, opts)
+    want_off, want_hits = best_filter(off_o, hits_o, opts[0], 1)
+    assert np.array_equal(off_g, want_off) and hits_g.tobytes() == want_hits.tobytes()
+    po_g, pairs_g, info = bc.bc_pair_batch(p.ix, res, d, 150, 450, 16)
+    po_o, pairs_o, sk = pair_reads(p.oracle.index(0)[0], want_off, want_hits, ln, 150, 450, 16)
+    assert np.array_equal(po_g, po_o) and pairs_g.tobytes() == pairs_o.tobytes() and info["skipped_hits"] == sk
