@@ -160,7 +160,7 @@ def run_ours(args):
     rank, world, local = bdist.init_from_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    dev = torch.device("cuda", local)
+    dev = torch.device("cuda", local % torch.cuda.device_count())   # (modulo only matters for the one-GPU plumbing test)
     torch.cuda.set_device(dev)
 
     cfg, desc = workload(args.config)
@@ -219,7 +219,7 @@ def run_ours(args):
         flush.fill_(1)
         one_step()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    sampler = ClockSampler(local) if rank == 0 else None
+    sampler = ClockSampler(dev.index) if rank == 0 else None
     bdist.barrier(); torch.cuda.synchronize()
     search_ns, stats = [], None
     for a, b in ev:

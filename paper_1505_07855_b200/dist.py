@@ -31,7 +31,8 @@ def init_from_env(backend: str | None = None):
         import torch
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29500")
-        be = backend or ("nccl" if torch.cuda.is_available() else "gloo")
+        # BC_DIST_BACKEND=gloo lets the N>1 plumbing be exercised where NCCL cannot run (several ranks on one GPU)
+        be = backend or os.environ.get("BC_DIST_BACKEND") or ("nccl" if torch.cuda.is_available() else "gloo")
         if be == "nccl":
             torch.cuda.set_device(local)
         _dist().init_process_group(backend=be, rank=rank, world_size=world)
