@@ -295,7 +295,16 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             uint32_t need = 32u - bcnt;
             unsigned long long tk = 0;
-            if (lane == 0) tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
+            if (lane == 0) {
+                // towards the end of the batch take fewer queries at a time, so that the last heavy
+                // trees are spread over the warps instead of queueing behind one another
+                const unsigned long long seen = *(volatile unsigned long long *)&ctr[BC_CTR_TICKET];
+                const unsigned long long left = seen < nq ? nq - seen : 0ull;
+                const unsigned long long fair = left / (4ull * gridDim.x * (blockDim.x >> 5)) + 1ull;
+                if (fair < need) need = (uint32_t)fair;
+                tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
+            }
+            need = __shfl_sync(0xffffffffu, need, 0);
             tk = __shfl_sync(0xffffffffu, tk, 0);
             if (tk + need >= nq) more = false;
             unsigned long long q = tk + lane;
