@@ -42,15 +42,17 @@ int choose_geometry(const bc_index *ix, const bc_opts *o, Geometry &g) {
     g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
     const uint32_t R = 8u * (uint32_t)o->z + 9u;
     for (;; --g.ctas) {
-        const size_t total_kb = 160;                  // leaves ~64 KB of the SM's 228 KB to L1 (index sectors, prep rows);
-                                                      // measured: 100/130/160/190/220 KB -> 146/126/116/117/131 ms on config 2
+        const size_t total_kb = 192;                  // leaves ~36 KB of the SM's 228 KB to L1 (index sectors, prep rows);
+                                                      // measured on config 2 (final kernel): 144/160/176/192/208/220 KB -> 101.5/98.0/96.7/95.5/98.1/99.1 ms
         size_t budget = total_kb * 1024 / g.ctas;
         if (budget > 200 * 1024) budget = 200 * 1024;
         uint32_t per_warp = (uint32_t)(budget / ((size_t)g.warps * BC_POOL_ENTRY_BYTES));
         if (per_warp > 4096) per_warp = 4096;
-        uint32_t bcap = 64;
-        while (bcap * 2 <= per_warp / 2) bcap *= 2;
-        while (bcap < 2 * R + 64 && bcap * 2 + 96 <= per_warp) bcap *= 2;     // deep budgets: a bigger ring
+        // the ring only has to hold the hot top of the branch stack (its bottom spills to global memory):
+        // 128 entries unless the budget is deep (a multi-lane step must leave it at <= bcap - R); the
+        // rest goes to the two chain stacks, which take ~120 pushes per 32-wide branch step
+        uint32_t bcap = per_warp >= 224 ? 128 : 64;
+        while (bcap < R + 64 && bcap * 2 + 96 <= per_warp) bcap *= 2;
         if (bcap >= R + 48 && per_warp >= bcap + 96) { g.bcap = bcap; g.ccap = per_warp - bcap; return BC_OK; }
         if (g.ctas == 1) return BC_E_UNSUPPORTED;     // z too large for the on-chip pool at this warp count
     }
