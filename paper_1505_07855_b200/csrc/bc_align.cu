@@ -42,8 +42,10 @@ int choose_geometry(const bc_index *ix, const bc_opts *o, Geometry &g) {
     g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
     const uint32_t R = 8u * (uint32_t)o->z + 9u;
     for (;; --g.ctas) {
-        const size_t total_kb = 192;                  // leaves ~36 KB of the SM's 228 KB to L1 (index sectors, prep rows);
-                                                      // measured on config 2 (final kernel): 144/160/176/192/208/220 KB -> 101.5/98.0/96.7/95.5/98.1/99.1 ms
+        // pool bytes per SM; what is left of the 228 KB stays L1 (index sectors, prep rows).  Measured with the
+        // final kernel: config 2 (16 MB index, L2-resident) 144/160/176/192/208/220 KB -> 101.5/98.0/96.7/95.5/
+        // 98.1/99.1 ms; configs 3 and 4 (index >= L2) are 2-3 % faster at 160 than at 192 (L2 misses make L1 count)
+        const size_t total_kb = ix->bytes > ((size_t)64 << 20) ? 160 : 192;
         size_t budget = total_kb * 1024 / g.ctas;
         if (budget > 200 * 1024) budget = 200 * 1024;
         uint32_t per_warp = (uint32_t)(budget / ((size_t)g.warps * BC_POOL_ENTRY_BYTES));
