@@ -43,6 +43,7 @@ def lib():
         L.orc_occ.restype = C.c_uint64
         L.orc_occ.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int64]
         L.orc_D.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.orc_D_range.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
         L.orc_locate.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
         L.orc_align.restype = C.c_void_p
         L.orc_align.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_int, C.c_int]
@@ -90,6 +91,13 @@ class Oracle:
         Q = np.ascontiguousarray(Q, dtype=np.uint8)
         out = np.empty(Q.size, np.int32)
         lib().orc_D(self._h, _ptr(Q), Q.size, _ptr(out))
+        return out
+
+    def D_range(self, Q, lo: int, hi: int) -> np.ndarray:
+        """Ds: the D loop restricted to Q[lo..hi); entries outside the range are 0."""
+        Q = np.ascontiguousarray(Q, dtype=np.uint8)
+        out = np.empty(Q.size, np.int32)
+        lib().orc_D_range(self._h, _ptr(Q), Q.size, lo, hi, _ptr(out))
         return out
 
     def locate(self, rows) -> np.ndarray:

@@ -288,6 +288,14 @@ void orc_D(void *hv, const uint8_t *Q, int m, int32_t *D) {
     for (int i = 0; i < m; ++i) D[i] = d[i];
 }
 
+// Ds[] ("Ds is the same loop started at i = s0 with cnt = 0"): the loop of orc_D restricted to
+// Q[from..to) -- an accessor for the pins, no arithmetic of its own.  Entries outside [from,to) are 0.
+void orc_D_range(void *hv, const uint8_t *Q, int m, int from, int to, int32_t *D) {
+    Handle *h = (Handle *)hv; std::vector<int> d(m, 0);
+    compute_D(h->rev, Q, from, to, d, nullptr);
+    for (int i = 0; i < m; ++i) D[i] = d[i];
+}
+
 // rows -> SA[row] (definition of locate)
 void orc_locate(void *hv, const uint32_t *rows, uint64_t n_rows, uint32_t *pos) {
     Handle *h = (Handle *)hv;
