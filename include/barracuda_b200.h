@@ -174,11 +174,18 @@ int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint3
  * [9] nodes expanded in branch steps, [10] warp-level chain iterations, [11] nodes expanded in
  * chain iterations, [12] branch states popped and put back because their children did not fit,
  * [13] 32-entry blocks of branch states spilled from the on-chip rings to the workspace,
- * [14..15] reserved. */
+ * [14] deepest per-warp spill stack seen (blocks), [15] passes (best-stratum mode). */
 int bc_last_stats(const bc_index *ix, uint64_t *out16);
 
 /* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM (<= 8), warps per CTA (<= 8). */
 int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
+
+/* More tuning (0 = default): spill_blocks = per-warp spill area of the branch rings in blocks of 32
+ * states (default 128; bc_align_batch returns BC_E_NOMEM when a warp's area runs full -- raise it, ask
+ * bc_align_workspace_bytes again and repeat the call); pool_kb = shared memory per SM given to the
+ * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond).  Affects the
+ * workspace size: set it before bc_align_workspace_bytes. */
+int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb);
 
 /* Host-side index construction for synthetic genomes (untimed helper): suffix sort
  * of T$ and reverse(T)$ -> transport arrays.  text: HOST, n codes 0..3.  The arrays are allocated

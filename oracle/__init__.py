@@ -38,6 +38,8 @@ def lib():
         L = C.CDLL(build())
         L.orc_index_build.restype = C.c_void_p
         L.orc_index_build.argtypes = [C.c_void_p, C.c_uint64, C.c_int]
+        L.orc_index_build2.restype = C.c_void_p
+        L.orc_index_build2.argtypes = [C.c_void_p, C.c_uint64, C.c_int, C.c_int]
         L.orc_index_free.argtypes = [C.c_void_p]
         L.orc_index_get.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_occ.restype = C.c_uint64
@@ -63,12 +65,15 @@ def _ptr(a):
 class Oracle:
     """Index of one genome (codes 0..3) + the reference search."""
 
-    def __init__(self, genome: np.ndarray, nthreads: int | None = None):
+    def __init__(self, genome: np.ndarray, nthreads: int | None = None, sort: str = "auto"):
+        """sort: "literal" (one comparison sort of all suffixes), "bucketed" (by the first 12
+        bases, then a comparison sort per bucket) or "auto" (literal up to 150 M suffixes)."""
         self.T = np.ascontiguousarray(genome, dtype=np.uint8)
         assert self.T.size == 0 or self.T.max() <= 3
         self.n = int(self.T.size)
         self.nthreads = nthreads or os.cpu_count() or 1
-        self._h = lib().orc_index_build(_ptr(self.T), self.n, self.nthreads)
+        mode = {"literal": 0, "bucketed": 1, "auto": -1}[sort]
+        self._h = lib().orc_index_build2(_ptr(self.T), self.n, self.nthreads, mode)
 
     def __del__(self):
         if getattr(self, "_h", None):

@@ -8,7 +8,8 @@
 // the other.  Integer arithmetic only; nothing here is tuned.
 //
 // What it follows (PAPER.md gives the method only in prose, so the contract is SURVEY.md 8c):
-//   * index: BWT by NAIVE SUFFIX SORT of T$ (north_star).  Two pointers k,l updated
+//   * index: BWT by NAIVE SUFFIX SORT of T$ (north_star; beyond 150 M suffixes the sort is
+//     bucketed by the first 12 bases and each bucket comparison-sorted, as C8 allows).  Two pointers k,l updated
 //     per base from the index, l-k+1 = number of matches, crossing = absent.
 //   * search: "carefully back up its search and start trying out alternatives" =
 //     the recursion of SURVEY C4, written out in that order and notation, on the alignment
@@ -72,12 +73,10 @@ struct SufLess {
     }
 };
 
-void build_index(Index &ix, const uint8_t *T, uint64_t n, int nthreads) {
-    ix.n = n; ix.T.assign(T, T + n);
-    ix.SA.resize(n + 1);
-    for (uint64_t i = 0; i <= n; ++i) ix.SA[i] = (uint32_t)i;
+// naive comparison sort of ALL suffixes; threads only split it into a merge sort
+void sort_suffixes_literal(Index &ix, int nthreads) {
+    const uint64_t n = ix.n;
     SufLess less{ix.T.data(), n};
-    // naive comparison sort of ALL suffixes; threads only split it into a merge sort
     int parts = 1; while (parts * 2 <= nthreads && (n + 1) / (parts * 2) > 4096) parts *= 2;
     std::vector<uint64_t> cut(parts + 1);
     for (int p = 0; p <= parts; ++p) cut[p] = (n + 1) * (uint64_t)p / parts;
@@ -96,10 +95,75 @@ void build_index(Index &ix, const uint8_t *T, uint64_t n, int nthreads) {
             });
         for (auto &t : th) t.join();
     }
+}
+
+// SURVEY C8, for genomes where the literal sort takes hours: "bucket suffixes by their first 12 bases
+// (16.7 M buckets), then comparison-sort each bucket on the text in parallel -- still no clever
+// construction algorithm".  Key of suffix i = its first 12 symbols, 2 bits each, padded with A (= 0) past
+// the end of T.  The padding cannot misplace a suffix ACROSS buckets: at the first position where two
+// padded prefixes differ, the suffix with the smaller symbol is the smaller suffix if that position lies
+// inside both, and a padded position (A, the smallest base) can never be the larger one.  WITHIN a bucket
+// the same literal comparator as above ('$' smallest) decides.  Pinned by equality with the literal sort
+// (tests/test_oracle_pins2.py).
+void sort_suffixes_bucketed(Index &ix, int nthreads) {
+    const uint64_t n = ix.n;
+    const int K = 12;
+    const uint64_t NB = 1ull << (2 * K);
+    const uint8_t *T = ix.T.data();
+    auto key_at = [&](uint64_t i) {            // suffix i = T[i..n) $ ; i == n is the '$' suffix: all padding
+        uint64_t key = 0;
+        for (int j = 0; j < K; ++j) key = (key << 2) | (i + j < n ? T[i + j] : 0);
+        return key;
+    };
+    std::vector<uint64_t> start(NB + 1, 0);
+    for (uint64_t i = 0; i <= n; ++i) start[key_at(i) + 1]++;
+    for (uint64_t b = 0; b < NB; ++b) start[b + 1] += start[b];
+    if (nthreads < 1) nthreads = 1;
+    // thread t owns the buckets [own[t], own[t+1]): about (n+1)/nthreads suffixes each
+    std::vector<uint64_t> own(nthreads + 1, NB);
+    own[0] = 0;
+    for (int t = 1; t < nthreads; ++t) {
+        const uint64_t want = (n + 1) * (uint64_t)t / nthreads;
+        own[t] = (uint64_t)(std::lower_bound(start.begin(), start.end(), want) - start.begin());
+        if (own[t] > NB) own[t] = NB;
+        if (own[t] < own[t - 1]) own[t] = own[t - 1];
+    }
+    SufLess less{T, n};
+    std::vector<std::thread> th;
+    for (int t = 0; t < nthreads; ++t)
+        th.emplace_back([&, t] {
+            const uint64_t b0 = own[t], b1 = own[t + 1];
+            if (b0 >= b1) return;
+            std::vector<uint64_t> fill(start.begin() + b0, start.begin() + b1);   // next free slot of my buckets
+            for (uint64_t i = 0; i <= n; ++i) {          // every thread scans the text, keeps what it owns
+                const uint64_t key = key_at(i);
+                if (key >= b0 && key < b1) ix.SA[fill[key - b0]++] = (uint32_t)i;
+            }
+            for (uint64_t b = b0; b < b1; ++b)
+                if (start[b + 1] - start[b] > 1) std::sort(ix.SA.begin() + start[b], ix.SA.begin() + start[b + 1], less);
+        });
+    for (auto &t : th) t.join();
+}
+
+// mode: 0 = literal sort of all suffixes, 1 = bucketed (C8), -1 = literal up to 150 M suffixes, bucketed beyond
+void build_index(Index &ix, const uint8_t *T, uint64_t n, int nthreads, int mode = 0) {
+    ix.n = n; ix.T.assign(T, T + n);
+    ix.SA.resize(n + 1);
+    for (uint64_t i = 0; i <= n; ++i) ix.SA[i] = (uint32_t)i;
+    if (mode == 1 || (mode < 0 && n > 150000000ull)) sort_suffixes_bucketed(ix, nthreads);
+    else sort_suffixes_literal(ix, nthreads);
     ix.B.resize(n + 1);
-    for (uint64_t j = 0; j <= n; ++j) {
-        if (ix.SA[j] == 0) { ix.B[j] = 4; ix.primary = j; }
-        else ix.B[j] = ix.T[ix.SA[j] - 1];
+    {                                            // B[j] = X[SA[j]-1]; threads only split the rows
+        const int nt = nthreads < 1 ? 1 : nthreads;
+        std::vector<std::thread> th;
+        for (int t = 0; t < nt; ++t)
+            th.emplace_back([&, t] {
+                for (uint64_t j = (n + 1) * (uint64_t)t / nt; j < (n + 1) * (uint64_t)(t + 1) / nt; ++j) {
+                    if (ix.SA[j] == 0) { ix.B[j] = 4; ix.primary = j; }
+                    else ix.B[j] = ix.T[ix.SA[j] - 1];
+                }
+            });
+        for (auto &t : th) t.join();
     }
     uint64_t cnt[4] = {0, 0, 0, 0};
     for (uint64_t i = 0; i < n; ++i) cnt[ix.T[i]]++;
@@ -258,13 +322,14 @@ void align_query(const Handle &h, const uint8_t *W, int m, const Opts &o, int fl
 
 extern "C" {
 
-void *orc_index_build(const uint8_t *T, uint64_t n, int nthreads) {
+void *orc_index_build2(const uint8_t *T, uint64_t n, int nthreads, int mode) {
     Handle *h = new Handle();
-    build_index(h->fwd, T, n, nthreads);
+    build_index(h->fwd, T, n, nthreads, mode);
     std::vector<uint8_t> R(T, T + n); std::reverse(R.begin(), R.end());
-    build_index(h->rev, R.data(), n, nthreads);
+    build_index(h->rev, R.data(), n, nthreads, mode);
     return h;
 }
+void *orc_index_build(const uint8_t *T, uint64_t n, int nthreads) { return orc_index_build2(T, n, nthreads, 0); }
 void orc_index_free(void *h) { delete (Handle *)h; }
 
 // which: 0 fwd, 1 rev.  Any out pointer may be NULL.

@@ -92,6 +92,7 @@ def lib():
         L.bc_locate.argtypes = [vp, vp, u64, vp, vp]
         L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 16)]
         L.bc_set_geometry.argtypes = [vp, u32, u32]
+        L.bc_set_tuning.argtypes = [vp, u32, u32]
         L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
         L.bc_index_build_gpu_bytes.argtypes = [u64, u32, u32, C.POINTER(C.c_size_t)]
@@ -100,7 +101,7 @@ def lib():
         L.bc_strerror.argtypes = [i32]
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
-                  "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_index_build_host",
+                  "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_set_tuning", "bc_index_build_host",
                   "bc_index_host_free", "bc_measure_random_sectors", "bc_align_best_workspace_bytes",
                   "bc_align_batch_best", "bc_pair_workspace_bytes", "bc_pair_batch", "bc_index_build_gpu_bytes", "bc_index_build_gpu"):
             getattr(L, f).restype = i32
@@ -224,6 +225,7 @@ class DeviceIndex:
 
     def __init__(self, handle, mem, n, device):
         self._h, self.mem, self.n, self.device = handle, mem, n, device
+        self.spill_blocks, self.pool_kb = 0, 0
 
     @property
     def handle(self):
@@ -268,8 +270,13 @@ def bc_set_geometry(ix: DeviceIndex, ctas_per_sm: int = 0, warps_per_cta: int = 
     _check(lib().bc_set_geometry(ix.handle, ctas_per_sm, warps_per_cta), "bc_set_geometry")
 
 
+def bc_set_tuning(ix: DeviceIndex, spill_blocks: int = 0, pool_kb: int = 0):
+    _check(lib().bc_set_tuning(ix.handle, spill_blocks, pool_kb), "bc_set_tuning")
+    ix.spill_blocks, ix.pool_kb = spill_blocks, pool_kb
+
+
 STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry",
-              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes", "cancelled", "spill_blocks", "reserved14", "passes")
+              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes", "cancelled", "spill_blocks", "spill_max", "passes")
 
 
 def bc_last_stats(ix: DeviceIndex) -> dict:
@@ -392,11 +399,16 @@ def bc_align_batch(ix: DeviceIndex, reads: DeviceReads, opts, ws: Workspace | No
     Returns (AlignResult, Workspace)."""
     if ws is None:
         ws = Workspace(ix, reads.n_reads, max(1, reads.max_len), opts)
-    for _ in range(4):
+    for _ in range(7):
         rc = bc_align_batch_raw(ix, reads, opts, ws, stream)
         if rc == BC_OK:
             need = ws.needed.cpu().numpy().view(np.uint64)
             return AlignResult(ws.hit_offsets, ws.hits, int(need[0]), int(need[1])), ws
+        if rc == BC_E_NOMEM and grow and (ix.spill_blocks or 128) < 8192:
+            # a warp's spill area of pending branch states ran full: give it more and repeat (never truncated)
+            bc_set_tuning(ix, 4 * (ix.spill_blocks or 128), ix.pool_kb)
+            ws = Workspace(ix, reads.n_reads, max(1, reads.max_len), opts, ws.raw_hits_per_read, ws.hits_capacity)
+            continue
         if rc != BC_E_OVERFLOW or not grow:
             raise BcError(rc, "bc_align_batch")
         need = ws.needed.cpu().numpy().view(np.uint64)

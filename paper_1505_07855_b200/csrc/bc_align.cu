@@ -11,52 +11,66 @@ constexpr uint64_t SCAN_TILE = 256 * 8;            // must match bc_post.cu
 constexpr size_t RAW_BYTES = sizeof(BcRawHit) + sizeof(uint64_t) + sizeof(uint32_t);   // arena + seg_key + seg_d
 
 struct WsLayout {
-    size_t off_prep, off_spill, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_ctr, fixed;
-    uint32_t stride, nq;
+    size_t off_qrec, off_spill, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_ctr, fixed;
+    uint32_t qstride, q_soff, q_boff, q_noff, nq, spill_blocks;
 };
 
-int make_ws_layout(uint32_t n_reads, uint32_t max_len, uint32_t grid_warps, WsLayout &L) {
+// the query record of bc_ws.cuh: thresholds | bases | N bits, 16-byte multiple
+void qrec_layout(const bc_opts *o, uint32_t max_len, bool with_n, WsLayout &L) {
+    const bool small = o->z <= BC_QREC_SMALL_Z && o->seed_z <= BC_QREC_SMALL_SZ;
+    L.q_soff = small ? 8u : (uint32_t)o->z + 1u;
+    L.q_boff = small ? 16u : (uint32_t)align_up((size_t)o->z + o->seed_z + 2, 16);
+    const uint32_t nb = (max_len / 16u + 1u) * 4u, nn = (max_len / 32u + 1u) * 4u;
+    L.q_noff = with_n ? L.q_boff + nb : 0u;
+    L.qstride = (uint32_t)align_up((size_t)L.q_boff + nb + (with_n ? nn : 0u), 16);
+}
+
+// the workspace is sized for a batch WITH an N mask (bc_align_workspace_bytes does not see the reads);
+// a batch without one uses the shorter records
+int make_ws_layout(uint32_t n_reads, uint32_t max_len, const bc_opts *o, bool with_n, uint32_t grid_warps,
+                   uint32_t spill_blocks, WsLayout &L) {
     if (max_len < 1 || max_len > BC_MAX_READ_LEN || n_reads > 0x7FFFFFF0u) return BC_E_INVAL;
     L.nq = 2 * n_reads;
-    L.stride = (max_len + 2) & ~1u;                // max_len + 1 entries, even so rows stay 4-byte aligned
-    size_t o = 0;
-    L.off_prep = o;    o = align_up(o + (size_t)L.nq * L.stride * 2, 256);
-    L.off_spill = o;   o = align_up(o + (size_t)grid_warps * BC_SPILL_BLOCKS * 32 * BC_POOL_ENTRY_BYTES, 256);
-    L.off_qcnt = o;    o = align_up(o + (size_t)L.nq * 4, 256);
-    L.off_qfill = o;   o = align_up(o + (size_t)L.nq * 4, 256);
-    L.off_seg_off = o; o = align_up(o + ((size_t)L.nq + 1) * 8, 256);
-    L.off_uoff = o;    o = align_up(o + ((size_t)L.nq + 1) * 8, 256);
-    L.off_blk = o;     o = align_up(o + ((size_t)L.nq / SCAN_TILE + 2) * 8, 256);
-    L.off_big = o;     o = align_up(o + (size_t)L.nq * 4, 256);
-    L.off_ctr = o;     o = align_up(o + BC_CTR_COUNT * 8, 256);
-    L.fixed = o;
+    L.spill_blocks = spill_blocks;
+    qrec_layout(o, max_len, true, L);
+    const size_t qrec_bytes = (size_t)L.nq * L.qstride;
+    qrec_layout(o, max_len, with_n, L);
+    size_t x = 0;
+    L.off_qrec = x;    x = align_up(x + qrec_bytes, 256);
+    L.off_spill = x;   x = align_up(x + (size_t)grid_warps * spill_blocks * 32 * BC_POOL_ENTRY_BYTES, 256);
+    L.off_qcnt = x;    x = align_up(x + (size_t)L.nq * 4, 256);
+    L.off_qfill = x;   x = align_up(x + (size_t)L.nq * 4, 256);
+    L.off_seg_off = x; x = align_up(x + ((size_t)L.nq + 1) * 8, 256);
+    L.off_uoff = x;    x = align_up(x + ((size_t)L.nq + 1) * 8, 256);
+    L.off_blk = x;     x = align_up(x + ((size_t)L.nq / SCAN_TILE + 2) * 8, 256);
+    L.off_big = x;     x = align_up(x + (size_t)L.nq * 4, 256);
+    L.off_ctr = x;     x = align_up(x + BC_CTR_COUNT * 8, 256);
+    L.fixed = x;
     return BC_OK;
 }
 
-struct Geometry { uint32_t ctas, warps, bcap, ccap; };
+struct Geometry { uint32_t ctas, warps, bcap, ccap, spill_blocks; };
 
 // geometry of the persistent kernel: CTAs per SM, warps per CTA, per-warp branch ring (power of two)
-// and chain stack sizes that fill the shared memory of an SM
-int choose_geometry(const bc_index *ix, const bc_opts *o, Geometry &g) {
+// and run-stack sizes that fill the shared memory given to the pools
+int choose_geometry(const bc_index *ix, Geometry &g) {
     g.warps = ix->warps_per_cta ? ix->warps_per_cta : 8;
     g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
-    const uint32_t R = 8u * (uint32_t)o->z + 9u;
+    g.spill_blocks = ix->spill_blocks ? ix->spill_blocks : BC_SPILL_BLOCKS;
     for (;; --g.ctas) {
-        // pool bytes per SM; what is left of the 228 KB stays L1 (index sectors, prep rows).  Measured with the
-        // final kernel: config 2 (16 MB index, L2-resident) 144/160/176/192/208/220 KB -> 101.5/98.0/96.7/95.5/
-        // 98.1/99.1 ms; configs 3 and 4 (index >= L2) are 2-3 % faster at 160 than at 192 (L2 misses make L1 count)
-        const size_t total_kb = ix->bytes > ((size_t)64 << 20) ? 160 : 192;
+        // pool bytes per SM; what is left of the 228 KB stays L1 (index sectors, query records).  Round 1, measured:
+        // config 2 (16 MB index, L2-resident) 144/160/176/192/208/220 KB -> 101.5/98.0/96.7/95.5/98.1/99.1 ms;
+        // configs 3 and 4 (index >= L2) 2-3 % faster at 160 than at 192 (L2 misses make L1 count)
+        const size_t total_kb = ix->pool_kb ? ix->pool_kb : (ix->bytes > ((size_t)64 << 20) ? 160 : 192);
         size_t budget = total_kb * 1024 / g.ctas;
         if (budget > 200 * 1024) budget = 200 * 1024;
         uint32_t per_warp = (uint32_t)(budget / ((size_t)g.warps * BC_POOL_ENTRY_BYTES));
         if (per_warp > 4096) per_warp = 4096;
-        // the ring only has to hold the hot top of the branch stack (its bottom spills to global memory):
-        // 128 entries unless the budget is deep (a multi-lane step must leave it at <= bcap - R); the
-        // rest goes to the two chain stacks, which take ~120 pushes per 32-wide branch step
-        uint32_t bcap = per_warp >= 224 ? 128 : 64;
-        while (bcap < R + 64 && bcap * 2 + 96 <= per_warp) bcap *= 2;
-        if (bcap >= R + 48 && per_warp >= bcap + 96) { g.bcap = bcap; g.ccap = per_warp - bcap; return BC_OK; }
-        if (g.ctas == 1) return BC_E_UNSUPPORTED;     // z too large for the on-chip pool at this warp count
+        // the ring only has to hold the hot top of the branch stack (its bottom spills to global memory in
+        // blocks of 32, kept >= 64 slots free): 128 entries; the rest goes to the two run stacks, which take
+        // most of the children of a 32-wide branch step
+        if (per_warp >= 128 + 96) { g.bcap = 128; g.ccap = per_warp - 128; return BC_OK; }
+        if (g.ctas == 1) return BC_E_UNSUPPORTED;     // too many warps per CTA for the on-chip pools
     }
 }
 
@@ -77,10 +91,10 @@ extern "C" int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, ui
     int rc = check_opts(o);
     if (rc) return rc;
     Geometry g;
-    rc = choose_geometry(ix, o, g);
+    rc = choose_geometry(ix, g);
     if (rc) return rc;
     WsLayout L;
-    rc = make_ws_layout(n_reads, max_len, (uint32_t)ix->sm_count * g.ctas * g.warps, L);
+    rc = make_ws_layout(n_reads, max_len, o, true, (uint32_t)ix->sm_count * g.ctas * g.warps, g.spill_blocks, L);
     if (rc) return rc;
     if (raw_hits_per_read == 0) raw_hits_per_read = 16;
     uint64_t cap = (uint64_t)raw_hits_per_read * n_reads + 1024;
@@ -107,10 +121,11 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     }
     if (!reads->bases2 || !reads->off || !reads->len) return BC_E_INVAL;
     Geometry g;
-    rc = choose_geometry(ix, o, g);
+    rc = choose_geometry(ix, g);
     if (rc) return rc;
     WsLayout L;
-    rc = make_ws_layout(reads->n_reads, reads->max_len, (uint32_t)ix->sm_count * g.ctas * g.warps, L);
+    rc = make_ws_layout(reads->n_reads, reads->max_len, o, reads->nmask != nullptr, (uint32_t)ix->sm_count * g.ctas * g.warps,
+                        g.spill_blocks, L);
     if (rc) return rc;
     if (ws_bytes < L.fixed + 3 * 256 + RAW_BYTES) return BC_E_NOMEM;
 
@@ -121,8 +136,8 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     p.o = *o;
     BcWorkspace &ws = p.ws;
     ws.nq = L.nq;
-    ws.stride = L.stride;
-    ws.prep = (uint16_t *)(base + L.off_prep);
+    ws.qrec = (uint8_t *)(base + L.off_qrec);
+    ws.qstride = L.qstride; ws.q_soff = L.q_soff; ws.q_boff = L.q_boff; ws.q_noff = L.q_noff;
     ws.qcnt = (uint32_t *)(base + L.off_qcnt);
     ws.qfill = (uint32_t *)(base + L.off_qfill);
     ws.seg_off = (uint64_t *)(base + L.off_seg_off);
@@ -143,7 +158,7 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     p.bcap = g.bcap;
     p.ccap = g.ccap;
     ws.spill = (uint2 *)(base + L.off_spill);
-    ws.spill_blocks = BC_SPILL_BLOCKS;
+    ws.spill_blocks = L.spill_blocks;
 
     cudaError_t e = cudaMemsetAsync(base + L.off_qcnt, 0, L.fixed - L.off_qcnt, st);   // qcnt .. ctr
     if (e == cudaSuccess) e = bc_launch_prepare(p, st);
@@ -151,8 +166,8 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     if (e == cudaSuccess) e = bc_launch_search(p, ix->sm_count, ctas, warps, st);
     if (e == cudaSuccess && ix->ev[1]) e = cudaEventRecord(ix->ev[1], st);
     if (e == cudaSuccess) e = bc_launch_post(p, *res, st);
-    uint64_t ctr[BC_CTR_COUNT];
-    if (e == cudaSuccess) e = cudaMemcpyAsync(ctr, ws.ctr, sizeof(ctr), cudaMemcpyDeviceToHost, st);
+    uint64_t *ctr = ix->h_ctr;                       // pinned: one asynchronous D2H, one synchronize per call
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctr, ws.ctr, BC_CTR_COUNT * sizeof(uint64_t), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { cudaGetLastError(); return BC_E_CUDA; }
 
@@ -172,20 +187,13 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     ix->stats[11] = ctr[BC_CTR_NODES] - ctr[BC_CTR_BNODES];
     ix->stats[12] = ctr[BC_CTR_CANCEL];
     ix->stats[13] = ctr[BC_CTR_SPILL];
+    ix->stats[14] = ctr[BC_CTR_SPILLMAX];
 
     if (ctr[BC_CTR_ERROR] & 1ull) return BC_E_INVAL;        // a read length outside 1..max_len
-    if (ctr[BC_CTR_ERROR] & 2ull) return BC_E_CUDA;         // pool bound violated: a bug, never silent
-    uint64_t needed[2] = {ctr[BC_CTR_TOTAL], ctr[BC_CTR_ARENA]};
-    if (ctr[BC_CTR_ARENA] > cap) {
-        needed[0] = 0;
-        if (cudaMemcpyAsync(res->n_hits_needed, needed, 16, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-            cudaStreamSynchronize(st) != cudaSuccess)
-            return BC_E_CUDA;
-        return BC_E_OVERFLOW;
-    }
-    if (cudaMemcpyAsync(res->n_hits_needed + 1, needed + 1, 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaStreamSynchronize(st) != cudaSuccess)
-        return BC_E_CUDA;
+    if (ctr[BC_CTR_ERROR] & 2ull) return BC_E_CUDA;         // pool discipline violated: a bug, never silent
+    if (ctr[BC_CTR_ERROR] & 4ull) return BC_E_NOMEM;        // a warp's spill area ran full: bc_set_tuning(more blocks)
+    // n_hits_needed[0..1] were written by the device (write_hits): {hits after dedup | 0 on arena overflow, raw hits}
+    if (ctr[BC_CTR_ARENA] > cap) return BC_E_OVERFLOW;
     if (ctr[BC_CTR_TOTAL] > res->hits_capacity) return BC_E_OVERFLOW;
     return BC_OK;
 }

@@ -140,7 +140,8 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
     ix->dev.sa_interval = h->sa_interval;
     ix->n = n;
     ix->bytes = L.total;
-    ix->ctas_per_sm = 0; ix->warps_per_cta = 0;
+    ix->ctas_per_sm = 0; ix->warps_per_cta = 0; ix->spill_blocks = 0; ix->pool_kb = 0;
+    ix->h_ctr = nullptr;
     for (int i = 0; i < 16; ++i) ix->stats[i] = 0;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -148,8 +149,10 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
     }
     ix->sm_count = sms;
     ix->ev[0] = ix->ev[1] = nullptr;
-    if (cudaEventCreate(&ix->ev[0]) != cudaSuccess || cudaEventCreate(&ix->ev[1]) != cudaSuccess) {
-        if (ix->ev[0]) cudaEventDestroy(ix->ev[0]);
+    if (cudaEventCreate(&ix->ev[0]) != cudaSuccess || cudaEventCreate(&ix->ev[1]) != cudaSuccess ||
+        cudaHostAlloc((void **)&ix->h_ctr, 32 * sizeof(uint64_t), cudaHostAllocDefault) != cudaSuccess) {
+        for (int i = 0; i < 2; ++i) if (ix->ev[i]) cudaEventDestroy(ix->ev[i]);
+        cudaGetLastError();
         delete ix; return BC_E_CUDA;
     }
     *out = ix;
@@ -159,6 +162,7 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
 extern "C" int bc_index_free(bc_index *ix) {
     if (!ix) return BC_E_INVAL;
     for (int i = 0; i < 2; ++i) if (ix->ev[i]) cudaEventDestroy(ix->ev[i]);
+    if (ix->h_ctr) cudaFreeHost(ix->h_ctr);
     delete ix;
     return BC_OK;
 }
@@ -184,6 +188,13 @@ extern "C" int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warp
     if (!ix || warps_per_cta > 8 || ctas_per_sm > 8) return BC_E_INVAL;
     ix->ctas_per_sm = ctas_per_sm;
     ix->warps_per_cta = warps_per_cta;
+    return BC_OK;
+}
+
+extern "C" int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb) {
+    if (!ix || spill_blocks > 65536 || (pool_kb != 0 && (pool_kb < 16 || pool_kb > 220))) return BC_E_INVAL;
+    ix->spill_blocks = spill_blocks;
+    ix->pool_kb = pool_kb;
     return BC_OK;
 }
 

@@ -42,10 +42,13 @@ struct bc_index {            // the opaque handle of the ABI
     BcIndexDev dev;
     uint64_t n;
     size_t bytes;
-    uint32_t ctas_per_sm, warps_per_cta;
+    uint32_t ctas_per_sm, warps_per_cta;   // 0 = chosen by the library (bc_set_geometry)
+    uint32_t spill_blocks;   // per-warp spill area of the branch rings, blocks of 32 states (bc_set_tuning)
+    uint32_t pool_kb;        // shared memory per SM given to the state pools, 0 = by index size (bc_set_tuning)
     uint64_t stats[16];
     int sm_count;
     cudaEvent_t ev[2];       // around the search kernel of the last bc_align_batch (stats[6])
+    uint64_t *h_ctr;         // pinned host copy of the device counter block (one D2H per call)
 };
 
 #ifdef __CUDACC__

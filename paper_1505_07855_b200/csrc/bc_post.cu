@@ -183,7 +183,8 @@ __global__ void sort_big(BcWorkspace ws) {
 __global__ void write_hits(BcWorkspace ws, bc_result res, uint32_t n_reads) {
     uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint64_t raw = ws.ctr[BC_CTR_ARENA], total = ws.uoff[ws.nq];
-    if (raw > ws.arena_cap) return;
+    if (i == 0) res.n_hits_needed[1] = raw;
+    if (raw > ws.arena_cap) { if (i == 0) res.n_hits_needed[0] = 0; return; }   // arena overflowed: nothing was sorted
     if (i == 0) { res.n_hits_needed[0] = total; ws.ctr[BC_CTR_TOTAL] = total; }
     if (i <= n_reads) res.hit_offsets[i] = ws.uoff[i < n_reads ? 2 * i : ws.nq];
     if (total > res.hits_capacity || i >= raw) return;

@@ -19,59 +19,68 @@ __device__ __forceinline__ uint32_t read_base(const bc_reads &rd, uint64_t pos) 
     return c;
 }
 
+// greedy piece count of SURVEY C7 over W[lo..hi), grown from W[hi-1] leftwards on the opposite-direction
+// index Y.  Whenever the count steps from c to c+1 at position a, D[a+1] = c is the last position with
+// D <= c: thr[c] = a+1 (thresholds beyond `rmax` are not needed; thr[] was zeroed: D[lo] <= r => 0).
+__device__ __forceinline__ void piece_thresholds(const bc_reads &rd, uint64_t off, uint32_t strand, const BcBwtDev &Y,
+                                                 int lo, int hi, int rmax, uint8_t *thr, uint64_t &lookups) {
+    const uint32_t full = Y.n + 1;
+    uint32_t cnt = 0, k = 0, s = full;
+    for (int a = hi - 1; a >= lo; --a) {
+        uint32_t c = read_base(rd, off + a);
+        if (c < 4 && strand) c = 3 - c;
+        bool brk = c > 3;
+        if (!brk) {
+            const uint32_t olo = bc_rank1(Y.lines, bc_rank_pos(Y, k), c), ohi = bc_rank1(Y.lines, bc_rank_pos(Y, k + s), c);
+            lookups += 2;
+            if (ohi == olo) brk = true; else { k = Y.C[c] + olo + 1; s = ohi - olo; }
+        }
+        if (brk) {
+            if ((int)cnt <= rmax) thr[cnt] = (uint8_t)(a + 1 < 255 ? a + 1 : 255);
+            cnt++; k = 0; s = full;
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
-// A1 + A2: one thread per query (read, strand).  SURVEY C7 loop, in W coordinates: pieces are
-// grown from W[m-1] leftwards by prepending on the opposite-direction index.
+// A1 + A2: one thread per query (read, strand): writes the query record of bc_ws.cuh -- bases
+// (complemented for strand 1), N bits, and the D / Ds bounds as thresholds.
 // ---------------------------------------------------------------------------------------------
 __global__ void bc_prepare_kernel(BcSearchParams p) {
     uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= p.ws.nq) return;
     uint32_t r = q >> 1, strand = q & 1;
     uint32_t m = p.reads.len[r];
-    uint16_t *out = p.ws.prep + (size_t)q * p.ws.stride;
+    uint8_t *rec = p.ws.qrec + (size_t)q * p.ws.qstride;
+    for (uint32_t i = 0; i < p.ws.qstride; i += 16) *reinterpret_cast<uint4 *>(rec + i) = make_uint4(0, 0, 0, 0);
     if (m < 1 || m > p.reads.max_len) {
         atomicOr((unsigned long long *)&p.ws.ctr[BC_CTR_ERROR], 1ull);
         return;
     }
     uint64_t off = p.reads.off[r];
+    // bases and N bits, re-aligned to bit 0 of the record's words
+    uint32_t *bw = reinterpret_cast<uint32_t *>(rec + p.ws.q_boff);
+    for (uint32_t w = 0; 16u * w < m; ++w) {
+        const uint64_t pos = off + 16u * w, last = off + (16u * w + 15u < m ? 16u * w + 15u : m - 1u);
+        const uint32_t lo = p.reads.bases2[pos >> 4], hi = (last >> 4) > (pos >> 4) ? p.reads.bases2[(pos >> 4) + 1] : 0u;
+        const uint32_t v = __funnelshift_r(lo, hi, 2u * (uint32_t)(pos & 15));
+        bw[w] = strand ? ~v : v;
+    }
+    if (p.ws.q_noff) {
+        uint32_t *nw = reinterpret_cast<uint32_t *>(rec + p.ws.q_noff);
+        for (uint32_t w = 0; 32u * w < m; ++w) {
+            const uint64_t pos = off + 32u * w, last = off + (32u * w + 31u < m ? 32u * w + 31u : m - 1u);
+            const uint32_t lo = p.reads.nmask[pos >> 5], hi = (last >> 5) > (pos >> 5) ? p.reads.nmask[(pos >> 5) + 1] : 0u;
+            uint32_t v = __funnelshift_r(lo, hi, (uint32_t)(pos & 31));
+            if (32u * w + 32u > m) v &= (1u << (m - 32u * w)) - 1u;   // bits past the read's end are not N
+            nw[w] = v;
+        }
+    }
     const BcBwtDev &Y = p.ix.bwt[strand ? 1 : 0];       // opposite direction of the search index
-    const uint32_t full = Y.n + 1;
     const bool seed_on = p.o.seed_len > 0 && (uint32_t)p.o.seed_len < m;
     uint64_t lookups = 0;
-    // pass 1: Ds over the seed part (entries outside the seed get 0 in pass 2)
-    if (seed_on) {
-        uint32_t cnt = 0, k = 0, s = full;
-        for (int a = p.o.seed_len - 1; a >= 0; --a) {
-            uint32_t c = read_base(p.reads, off + a);
-            if (c < 4 && strand) c = 3 - c;
-            if (c > 3) { cnt++; k = 0; s = full; }
-            else {
-                uint32_t olo = bc_rank1(Y.lines, bc_rank_pos(Y, k), c), ohi = bc_rank1(Y.lines, bc_rank_pos(Y, k + s), c);
-                lookups += 2;
-                uint32_t s2 = ohi - olo;
-                if (s2 == 0) { cnt++; k = 0; s = full; } else { k = Y.C[c] + olo + 1; s = s2; }
-            }
-            out[a] = (uint16_t)((cnt < 63 ? cnt : 63) << 9);
-        }
-    }
-    // pass 2: D over the whole read + the consumed base
-    {
-        uint32_t cnt = 0, k = 0, s = full;
-        for (int a = (int)m - 1; a >= 0; --a) {
-            uint32_t c = read_base(p.reads, off + a);
-            if (c < 4 && strand) c = 3 - c;
-            if (c > 3) { cnt++; k = 0; s = full; }
-            else {
-                uint32_t olo = bc_rank1(Y.lines, bc_rank_pos(Y, k), c), ohi = bc_rank1(Y.lines, bc_rank_pos(Y, k + s), c);
-                lookups += 2;
-                uint32_t s2 = ohi - olo;
-                if (s2 == 0) { cnt++; k = 0; s = full; } else { k = Y.C[c] + olo + 1; s = s2; }
-            }
-            uint32_t ds = (seed_on && a < p.o.seed_len) ? (out[a] & (63u << 9)) : 0u;
-            out[a] = (uint16_t)(c | ((cnt < 63 ? cnt : 63) << 3) | ds);
-        }
-        out[m] = 0;
-    }
+    if (seed_on) piece_thresholds(p.reads, off, strand, Y, 0, p.o.seed_len, p.o.seed_z, rec + p.ws.q_soff, lookups);
+    piece_thresholds(p.reads, off, strand, Y, 0, (int)m, p.o.z, rec, lookups);
     atomicAdd((unsigned long long *)&p.ws.ctr[BC_CTR_DLOOKUPS], (unsigned long long)lookups);
 }
 
@@ -94,9 +103,10 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 // Pool entry = 24 bytes, array-of-structures, moved with three 64-bit shared-memory accesses:
 //   {qid, k} {s, k2} {mlo, mhi}
 //   mlo = t (bits 0-8) | st (9-10; 0 = M, 1 = I, 2 = D) | n_go (11-18) | n_ge (19-26)
-//   mhi = seed_d (0-7) | d (8-15) | m-1 (16-23);  chain entries also carry their next base in mlo bits 27-29
-// Per warp: a RING of BRANCH states (budget left, d < z), whose cold bottom spills to global memory in
-// blocks of 32, and a stack of CHAIN states (budget exhausted, d == z: only exact matching follows).
+//   mhi = seed_d (0-7) | d (8-15) | m-1 (16-23)
+//   run entries also carry the base they match next (mlo bits 27-29) and the end of their run - 1 (mhi 24-31)
+// Per warp: a RING of BRANCH states (some difference is affordable at their position), whose cold bottom
+// spills to global memory in blocks of 32, and two stacks of RUN states (see the kernel's comment).
 #ifndef BC_SEARCH_MAX_THREADS
 #define BC_SEARCH_MAX_THREADS 256
 #endif
@@ -146,27 +156,77 @@ __device__ __noinline__ void flush_stats(unsigned long long *ctr, uint32_t lane,
     }
 }
 
-struct SearchConsts {            // warp-uniform values the phases share; suffix = strand
-    const uint4 *lines0, *lines1;   // index the strand's query is matched on (strand 0: reverse index)
-    uint32_t primary0, primary1;
-};
+// ---- query record access (layout in bc_ws.cuh) ------------------------------------------------
+struct QThr { uint32_t dlo, dhi, s; const uint8_t *rec; };
+
+template <bool SMALL>
+__device__ __forceinline__ QThr load_thr(const uint8_t *rec) {
+    QThr q; q.rec = rec; q.dlo = q.dhi = q.s = 0;
+    if (SMALL) { const uint4 v = __ldg(reinterpret_cast<const uint4 *>(rec)); q.dlo = v.x; q.dhi = v.y; q.s = v.z; }
+    return q;
+}
+template <bool SMALL>
+__device__ __forceinline__ uint32_t thr_d(const QThr &q, int r) {             // smallest t with D[t] <= r
+    if (SMALL) return __byte_perm(q.dlo, q.dhi, (uint32_t)r) & 255u;
+    return __ldg(q.rec + r);
+}
+template <bool SMALL>
+__device__ __forceinline__ uint32_t thr_s(const QThr &q, int r, uint32_t soff) {   // ... with Ds[t] <= r
+    if (SMALL) return (q.s >> (8u * (uint32_t)r)) & 255u;
+    return __ldg(q.rec + soff + r);
+}
+template <bool HAS_N>
+__device__ __forceinline__ uint32_t q_base(const uint8_t *rec, uint32_t boff, uint32_t noff, uint32_t t) {
+    const uint32_t w = __ldg(reinterpret_cast<const uint32_t *>(rec + boff) + (t >> 4));
+    uint32_t c = (w >> (2u * (t & 15u))) & 3u;
+    if (HAS_N) {
+        const uint32_t nm = __ldg(reinterpret_cast<const uint32_t *>(rec + noff) + (t >> 5));
+        if ((nm >> (t & 31u)) & 1u) c = 4u;
+    }
+    return c;
+}
+
+// First position at which a state with d = dc, seed differences sdc can afford ANY difference: before it
+// the D / Ds bounds (or a spent seed budget) leave exact matching as the only move.  dc == z: the read's end.
+// A value that is too SMALL only sends the state to a branch step early, which applies every rule itself.
+//   mismatch / insertion at t need D[t+1] <= z-dc-1, i.e. t >= thrD[z-dc-1] - 1 (deletions one later);
+//   inside the seed also sdc < seed_z and Ds[t+1] <= seed_z-sdc-1.
+// With E == 0 a deletion may precede W[0] outside the seed rule and follow W[m-1]; runs are then used for
+// spent budgets only (tests only; every config has E = 5).
+template <bool SMALL>
+__device__ __forceinline__ uint32_t run_end(const QThr &q, int dc, int sdc, int z, int seed_z, bool seed_on,
+                                            uint32_t seed_len, uint32_t m, bool e0, uint32_t soff) {
+    if (dc >= z) return m;
+    if (e0) return 0u;
+    uint32_t te = thr_d<SMALL>(q, z - dc - 1);
+    te = te ? te - 1u : 0u;
+    if (seed_on) {
+        uint32_t ts = seed_len;
+        if (sdc < seed_z) { ts = thr_s<SMALL>(q, seed_z - sdc - 1, soff); ts = ts ? ts - 1u : 0u; }
+        te = te > ts ? te : ts;
+    }
+    return te;
+}
 
 // ---------------------------------------------------------------------------------------------
-// CHAIN steps (see the kernel's header comment): while the stack of strand S holds a warp's worth
-// of chain states (or, when draining, anything at all), pop 32, extend each by ONE exactly matching
-// base -- one symbol's rank at both interval ends -- and push the survivors back compacted.  Flat
-// cost per node whatever the chain lengths; lanes are full whenever 32 states are pending.
+// RUN steps (see the kernel's header comment): while the stack of strand S holds a warp's worth of run
+// states (or, when draining, anything at all), pop 32, extend each by ONE exactly matching base -- one
+// symbol's rank at both interval ends -- and push the survivors back compacted.  A state whose run ends
+// (t == its run end) is a hit if the read is consumed, else it moves to the branch ring.  Flat cost per
+// node whatever the run lengths; lanes are full whenever 32 states are pending.
 // Strand 0 (searched on the reverse index) also advances the forward interval start k2 by the
 // bidirectional update of SURVEY C7 (R): '$' + the symbols smaller than c inside the interval.
-// Stack layout inside the chain area Cq[0..CCAP): strand 1 grows up from 0, strand 0 down from CCAP-1.
+// Stack layout inside the run area Cq[0..CCAP): strand 1 grows up from 0, strand 0 down from CCAP-1.
+// The caller guarantees 32 free ring slots per iteration (the loop re-checks).
 // ---------------------------------------------------------------------------------------------
-template <bool S0>
+template <bool S0, bool HAS_N>
 __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4 *lines, uint32_t primary,
                                             const uint32_t *Cs, uint2 *Cq, uint32_t CCAP, uint32_t &cnt,
-                                            bool drain, unsigned long long *ctr, uint32_t &n_nodes, uint32_t &n_xsect,
+                                            bool drain, uint2 *P, uint32_t bb, uint32_t &bcnt, uint32_t BCAP,
+                                            unsigned long long *ctr, uint32_t &n_nodes, uint32_t &n_xsect,
                                             uint32_t &n_steps) {
-    const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u;
-    while (cnt >= 32u || (drain && cnt > 0u)) {
+    const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u, BM = BCAP - 1u;
+    while ((cnt >= 32u || (drain && cnt > 0u)) && bcnt + 32u <= BCAP) {
         const uint32_t a = cnt < 32u ? cnt : 32u;
         const bool act = lane < a;
         uint32_t qid = 0, k = 0, s = 0, k2 = 0, mlo = 0, mhi = 0;
@@ -179,8 +239,8 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
         __syncwarp();
         n_nodes += a; ++n_steps;
         uint32_t t = mlo & 511u;
-        const uint32_t c = mlo >> 27, m = ((mhi >> 16) & 255u) + 1u;
-        bool alive = false, emit = false;
+        const uint32_t c = (mlo >> 27) & 7u, m = ((mhi >> 16) & 255u) + 1u, te = (mhi >> 24) + 1u;
+        bool alive = false, emit = false, toring = false;
         if (act) {
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
@@ -208,17 +268,22 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
                     k2 = c == 0u ? k2 + dollar : (c == 1u ? k2 + dollar + nx : (c == 2u ? k2 + s - nx - nc_ : k2 + s - nc_));
                 }
                 k = Cs[c] + olo + 1u; s = ohi - olo; ++t;
-                emit = t == m; alive = !emit;
+                const bool done = t == te;
+                emit = done && t == m; toring = done && !emit; alive = !done;
             }
         }
         uint32_t nb = 0;
-        if (alive) nb = BC_PREP_BASE(p.ws.prep[(size_t)qid * p.ws.stride + t]);
+        if (alive) nb = q_base<HAS_N>(p.ws.qrec + (size_t)qid * p.ws.qstride, p.ws.q_boff, p.ws.q_noff, t);
         const uint32_t smask = __ballot_sync(0xffffffffu, alive);
         if (alive) {
             const uint32_t r = __popc(smask & lt_mask);
-            ent_store(Cq, S0 ? CCAP - 1u - cnt - r : cnt + r, qid, k, s, k2, t | (nb << 27), mhi);
+            ent_store(Cq, S0 ? CCAP - 1u - cnt - r : cnt + r, qid, k, s, k2, (mlo & 0x07FFFE00u) | t | (nb << 27), mhi);
         }
         cnt += __popc(smask);
+        const uint32_t rmask = __ballot_sync(0xffffffffu, toring);
+        if (toring)      // a run consists of matches: gap state M, budgets unchanged
+            ent_store(P, (bb + bcnt + __popc(rmask & lt_mask)) & BM, qid, k, s, k2, (mlo & 0x07FFF800u) | t, mhi & 0x00FFFFFFu);
+        bcnt += __popc(rmask);
         if (__any_sync(0xffffffffu, emit))
             emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, S0 ? k2 : k, s, (mhi >> 8) & 255u);
         __syncwarp();
@@ -226,59 +291,61 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
 }
 
 // ---------------------------------------------------------------------------------------------
-// A3 + A4 + A5.  Persistent kernel, one LIFO pool per warp, two kinds of step:
+// A3 + A4 + A5.  Persistent kernel, one LIFO pool per warp, two kinds of state and of step:
 //  * BRANCH step: up to 32 branch states are popped, one per lane, and expanded in lock step:
 //    all four child intervals from one rank4 pair (1-2 index sectors) -> match, <=3 mismatch,
 //    <=4 deletion and 1 insertion children, pruned by the budgets and D/Ds.  Every lane counts its
-//    surviving children, a warp scan assigns pool slots, and each lane writes its own children:
-//    those that still have budget to the branch stack (match child deepest), those with d == z to
-//    the chain stack; terminal children are emitted.
-//  * CHAIN steps: whenever a strand's chain stack holds 32 states, 32 are popped, each is extended
-//    by ONE exactly matching base (one symbol's rank at both interval ends) and the survivors are
-//    pushed back compacted -- a flat cost per node, full lanes, whatever the chain lengths.
+//    surviving children, a warp scan assigns pool slots, and each lane writes its own children.
+//  * RUN steps: a state that can afford no difference before position `te` -- its budget is spent
+//    (te = m), its seed budget is spent (te = seed_len), or the D / Ds bounds say so -- can only match
+//    exactly until there.  Such states live on two stacks (one per strand); whenever a stack holds 32,
+//    32 are popped and each is extended by ONE exactly matching base (one symbol's rank at both interval
+//    ends); survivors go back compacted, finished runs are emitted (t == m) or become branch states.
+//    Flat cost per node, full lanes, whatever the run lengths.
 // New queries are drawn from a global ticket counter whenever fewer than 32 branch states are
 // pending, so lanes stay busy and converged whatever the shape of the individual search trees.
-// Pool bound: a multi-lane step keeps only the leading lanes whose children leave the
-// ring at <= BCAP - R entries (R = 8z+9) and fit the chain stack; the others are un-popped.  Lane 0
-// alone may fill the ring up to BCAP, and a run of single-lane steps from height P <= BCAP - R never
-// exceeds P-1+R because the match child is explored last.  If even lane 0 does not fit, the chain
-// stack (which only shrinks) is drained first.  Spilling the ring's bottom to global memory is an
-// optimisation on top of that bound (it keeps steps 32 wide), not part of it.
+// Pool discipline: a multi-lane branch step keeps only the leading lanes whose children fit the ring
+// and the run stacks; the others are un-popped (their entries are still in place).  The ring's cold
+// bottom moves to a per-warp area of the workspace in blocks of 32 whenever fewer than 64 slots are
+// free and comes back when the ring runs low; if that area is ever full the warp raises error bit 2
+// (BC_E_NOMEM: the caller passes a larger spill area), never a silent truncation.
 // ---------------------------------------------------------------------------------------------
+template <bool SMALL, bool HAS_N>
 __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
     uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
-    uint2 *Cq = P + 3u * BCAP;                                    // chain area: strand 1 up from 0, strand 0 down from CCAP-1
+    uint2 *Cq = P + 3u * BCAP;                                    // run area: strand 1 up from 0, strand 0 down from CCAP-1
     uint2 *G = p.ws.spill + ((size_t)blockIdx.x * (blockDim.x >> 5) + warp) * ((size_t)p.ws.spill_blocks * 96u);
     const uint32_t GB = p.ws.spill_blocks;
     const uint32_t lt_mask = (1u << lane) - 1u;
     const int z = p.o.z, E = p.o.indel_end_skip, max_go = p.o.max_gap_open, max_ge = p.o.max_gap_ext;
     const int seed_len = p.o.seed_len, seed_z = p.o.seed_z;
-    const uint32_t R = 8u * (uint32_t)z + 9u;
+    const bool e0 = E == 0;
     const uint32_t nq = p.ws.nq;
     const uint32_t full = p.ix.bwt[0].n + 1;
+    const uint32_t qstride = p.ws.qstride, soff = p.ws.q_soff, boff = p.ws.q_boff, noff = p.ws.q_noff;
     unsigned long long *ctr = (unsigned long long *)p.ws.ctr;
-    SearchConsts sc;
-    sc.lines0 = p.ix.bwt[1].lines; sc.lines1 = p.ix.bwt[0].lines;          // strand 0 searches the reverse index
-    sc.primary0 = p.ix.bwt[1].primary; sc.primary1 = p.ix.bwt[0].primary;
+    const uint4 *lines0 = p.ix.bwt[1].lines, *lines1 = p.ix.bwt[0].lines;  // strand 0 searches the reverse index
+    const uint32_t primary0 = p.ix.bwt[1].primary, primary1 = p.ix.bwt[0].primary;
 
     if (threadIdx.x < 8) Ctab[threadIdx.x] = p.ix.bwt[threadIdx.x < 4 ? 1 : 0].C[threadIdx.x & 3];
     __syncthreads();
-    uint32_t bb = 1u << 24, bcnt = 0, c0 = 0, c1 = 0, gsp = 0, pool_max = 0;   // ring bottom, counts (branch, chain per strand), spilled blocks
+    uint32_t bb = 1u << 24, bcnt = 0, c0 = 0, c1 = 0, gsp = 0, gsp_max = 0, pool_max = 0;   // ring bottom, counts (branch, run per strand), spilled blocks
     bool more = true, force_drain = false;
     // 32-bit statistics, flushed to the 64-bit global counters at every intake and at the end
     uint32_t n_cnodes = 0, n_xsect = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0, n_cancel = 0, n_spill = 0;
 
     for (;;) {
-        // ---- ring <-> global: keep the hot top of the branch stack on chip --------------------------
-        while (bcnt >= 64u && bcnt + 96u + R > BCAP && gsp < GB) {          // spill the bottom 32 entries
+        // ---- ring <-> global: keep the hot top of the branch stack on chip, >= 64 slots free ----------
+        while (bcnt >= 32u && bcnt + 64u > BCAP && gsp < GB) {               // spill the bottom 32 entries
             const uint2 *src = P + ((bb + lane) & BM) * 3u;
             uint2 *dst = G + ((size_t)gsp * 32u + lane) * 3u;
             dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
             bb += 32u; bcnt -= 32u; ++gsp; ++n_spill;
+            gsp_max = gsp > gsp_max ? gsp : gsp_max;
             __syncwarp();
         }
         if (bcnt < 32u && gsp > 0u) {                                          // bring the last block back
@@ -309,30 +376,39 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             if (tk + need >= nq) more = false;
             unsigned long long q = tk + lane;
             bool ok = lane < need && q < nq;
-            uint32_t m = 0, pr = 0;
+            uint32_t m = 0, te = 0, b0 = 0;
             if (ok) {
                 m = p.reads.len[q >> 1];
-                pr = p.ws.prep[(size_t)q * p.ws.stride];
-                ok = m >= 1 && m <= p.reads.max_len && (int)BC_PREP_D(pr) <= z && (int)BC_PREP_DS(pr) <= seed_z;
+                ok = m >= 1 && m <= p.reads.max_len;
             }
-            const bool odd = (q & 1ull) != 0;
-            const uint32_t mask = __ballot_sync(0xffffffffu, ok);
-            const uint32_t mask1 = __ballot_sync(0xffffffffu, ok && odd), mask0 = mask & ~mask1;
             if (ok) {
-                if (z > 0) ent_store(P, (bb + bcnt + __popc(mask & lt_mask)) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
-                else ent_store(Cq, odd ? c1 + __popc(mask1 & lt_mask) : CCAP - 1u - c0 - __popc(mask0 & lt_mask), (uint32_t)q,
-                               0u, full, 0u, BC_PREP_BASE(pr) << 27, (m - 1) << 16);
+                const uint8_t *rec = p.ws.qrec + (size_t)q * qstride;
+                const QThr th = load_thr<SMALL>(rec);
+                const bool seed_on = seed_len > 0 && seed_len < (int)m;
+                // D[0] <= z and Ds[0] <= seed_z, else nothing can align
+                ok = thr_d<SMALL>(th, z) == 0u && (!seed_on || thr_s<SMALL>(th, seed_z, soff) == 0u);
+                te = run_end<SMALL>(th, 0, 0, z, seed_z, seed_on, (uint32_t)seed_len, m, e0, soff);
+                b0 = q_base<HAS_N>(rec, boff, noff, 0u);
             }
-            if (z > 0) bcnt += __popc(mask); else { c1 += __popc(mask1); c0 += __popc(mask0); }
+            const bool odd = (q & 1ull) != 0, run = ok && te > 0u;
+            const uint32_t maskb = __ballot_sync(0xffffffffu, ok && !run);
+            const uint32_t mask1 = __ballot_sync(0xffffffffu, run && odd), mask0 = __ballot_sync(0xffffffffu, run && !odd);
+            if (ok) {
+                if (!run) ent_store(P, (bb + bcnt + __popc(maskb & lt_mask)) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
+                else ent_store(Cq, odd ? c1 + __popc(mask1 & lt_mask) : CCAP - 1u - c0 - __popc(mask0 & lt_mask), (uint32_t)q,
+                               0u, full, 0u, b0 << 27, ((m - 1) << 16) | ((te - 1u) << 24));
+            }
+            bcnt += __popc(maskb); c1 += __popc(mask1); c0 += __popc(mask0);
             __syncwarp();
         }
         if (bcnt == 0 && c0 + c1 == 0) { if (!more) break; continue; }
         pool_max = bcnt + c0 + c1 > pool_max ? bcnt + c0 + c1 : pool_max;
 
         if (c1 >= 32u || c0 >= 32u || ((bcnt == 0 || force_drain) && c0 + c1 > 0u)) {
+            if (bcnt + 32u > BCAP) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 4ull); break; }   // spill area exhausted
             const bool drain = bcnt == 0 || force_drain;
-            chain_steps<false>(p, sc.lines1, sc.primary1, Ctab + 4, Cq, CCAP, c1, drain, ctr, n_cnodes, n_xsect, n_csteps);
-            chain_steps<true>(p, sc.lines0, sc.primary0, Ctab, Cq, CCAP, c0, drain, ctr, n_cnodes, n_xsect, n_csteps);
+            chain_steps<false, HAS_N>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
+            chain_steps<true, HAS_N>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
             force_drain = false;
             continue;
         }
@@ -355,23 +431,23 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         const bool has_base = act && t < m;
         const bool del_ok = act && st != 1 && t >= E && m - t >= E;
         const bool ins_ok = has_base && st != 2 && t >= E && m - 1 - t >= E;
-        uint32_t pr0 = 0, pr1 = 0;
-        if (act) {
-            const uint16_t *pp = p.ws.prep + (size_t)qid * p.ws.stride + t;
-            pr0 = pp[0];
-            if (has_base) pr1 = pp[1];
+        const uint8_t *rec = p.ws.qrec + (size_t)qid * qstride;
+        QThr th = load_thr<SMALL>(act ? rec : p.ws.qrec);
+        uint32_t qb = 4u, qb1 = 4u;                      // W[t], W[t+1] of the query (4 = N / none)
+        if (has_base) {
+            qb = q_base<HAS_N>(rec, boff, noff, (uint32_t)t);
+            if (t + 1 < m) qb1 = q_base<HAS_N>(rec, boff, noff, (uint32_t)t + 1u);
         }
-        const uint32_t qb = BC_PREP_BASE(pr0);
         uint32_t nk[4] = {0, 0, 0, 0}, ns[4] = {0, 0, 0, 0}, nk2[4] = {0, 0, 0, 0};
         bool straddle = false;
         if (has_base || del_ok) {
-            const uint4 *lines = strand ? sc.lines1 : sc.lines0;
-            const uint32_t primary = strand ? sc.primary1 : sc.primary0;
+            const uint4 *lines = strand ? lines1 : lines0;
+            const uint32_t primary = strand ? primary1 : primary0;
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             uint32_t olo[4], ohi[4];
             bc_rank4(lines, plo, olo);                    // two unconditional loads: predicating the second one on
-            bc_rank4(lines, phi, ohi);                    // "other sector" was measured 3 % slower here (not in the chain step)
+            bc_rank4(lines, phi, ohi);                    // "other sector" was measured 3 % slower here (not in the run step)
             straddle = (plo >> 6) != (phi >> 6);
             const uint4 Cv = *reinterpret_cast<const uint4 *>(Ctab + strand * 4u);
             const uint32_t Cc[4] = {Cv.x, Cv.y, Cv.z, Cv.w};
@@ -384,23 +460,31 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         const int in_seed_base = (seed_on && t < seed_len) ? 1 : 0;
         const int in_seed_del = (seed_on && t > 0 && t < seed_len) ? 1 : 0;
         const uint32_t m_bits = mhi & 0x00FF0000u;
-        // class-level validity and packed child state (same for every child of a class)
-        const int nd1 = d + 1;
-        const bool v_mm = has_base && nd1 <= z && sd + in_seed_base <= seed_z && z - nd1 >= (int)BC_PREP_D(pr1) &&
-                          seed_z - (sd + in_seed_base) >= (int)BC_PREP_DS(pr1);
-        const int d_go = go + (st != 2), d_ge = ge + (st == 2), i_go = go + (st != 1), i_ge = ge + (st == 1);
-        const bool v_del = del_ok && nd1 <= z && d_go <= max_go && d_ge <= max_ge && sd + in_seed_del <= seed_z &&
-                           z - nd1 >= (int)BC_PREP_D(pr0) && seed_z - (sd + in_seed_del) >= (int)BC_PREP_DS(pr0);
-        const bool v_ins = ins_ok && nd1 <= z && i_go <= max_go && i_ge <= max_ge && sd + in_seed_base <= seed_z &&
-                           z - nd1 >= (int)BC_PREP_D(pr1) && seed_z - (sd + in_seed_base) >= (int)BC_PREP_DS(pr1);
+        // class-level validity and packed child state (same for every child of a class).  A child that costs a
+        // difference has d+1 = nd1 and needs D <= z - nd1 at ITS position: t+1 for mismatch / insertion, t for a
+        // deletion; inside the seed the same with Ds and the seed budget (zero thresholds outside / seed off).
+        const int nd1 = d + 1, sdb = sd + in_seed_base, sdd = sd + in_seed_del;
         const uint32_t tn = (uint32_t)t + 1u;
+        const bool bud = act && nd1 <= z;
+        const uint32_t thD = bud ? thr_d<SMALL>(th, z - nd1) : 0u;
+        const bool v_base = bud && has_base && sdb <= seed_z && tn >= thD && tn >= thr_s<SMALL>(th, sdb <= seed_z ? seed_z - sdb : 0, soff);
+        const int d_go = go + (st != 2), d_ge = ge + (st == 2), i_go = go + (st != 1), i_ge = ge + (st == 1);
+        const bool v_mm = v_base;
+        const bool v_ins = v_base && ins_ok && i_go <= max_go && i_ge <= max_ge;
+        const bool v_del = bud && del_ok && d_go <= max_go && d_ge <= max_ge && sdd <= seed_z && (uint32_t)t >= thD &&
+                           (uint32_t)t >= thr_s<SMALL>(th, sdd <= seed_z ? seed_z - sdd : 0, soff);
+        // where the children go: the end of the run a child starts with (te > its position: run stack)
+        const uint32_t te_b = run_end<SMALL>(th, nd1, sdb, z, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
+        const uint32_t te_d = in_seed_del == in_seed_base ? te_b
+                              : run_end<SMALL>(th, nd1, sdd, z, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
+        const bool run_b = te_b > tn, run_d = te_d > (uint32_t)t;
         const uint32_t ma_lo = tn | ((uint32_t)go << 11) | ((uint32_t)ge << 19);
         const uint32_t ma_hi = (uint32_t)sd | ((uint32_t)d << 8) | m_bits;
-        const uint32_t mm_hi = (uint32_t)(sd + in_seed_base) | ((uint32_t)nd1 << 8) | m_bits;
+        const uint32_t mm_hi = (uint32_t)sdb | ((uint32_t)nd1 << 8) | m_bits | (run_b ? (te_b - 1u) << 24 : 0u);
         const uint32_t de_lo = (uint32_t)t | (2u << 9) | ((uint32_t)d_go << 11) | ((uint32_t)d_ge << 19);
-        const uint32_t de_hi = (uint32_t)(sd + in_seed_del) | ((uint32_t)nd1 << 8) | m_bits;
+        const uint32_t de_hi = (uint32_t)sdd | ((uint32_t)nd1 << 8) | m_bits | (run_d ? (te_d - 1u) << 24 : 0u);
         const uint32_t in_lo = tn | (1u << 9) | ((uint32_t)i_go << 11) | ((uint32_t)i_ge << 19);
-        const uint32_t cb0 = qb << 27, cb1 = BC_PREP_BASE(pr1) << 27;   // first base of a chain child (bits 27-29)
+        const uint32_t cb0 = run_d ? qb << 27 : 0u, cb1 = run_b ? qb1 << 27 : 0u;   // first base of a run child
         const bool last1 = nd1 == z;                     // children that cost a difference exhaust the budget
         const bool term_base = (int)tn == m;             // children that consume W[t] finish the read
         const bool term_del = t == m;
@@ -419,12 +503,12 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         uint32_t ebits = vbits & tbits;
         if (s == full) ebits &= ~512u;                   // the empty string is not a hit (C3)
         // a terminal state is expanded further only for trailing deletions (E == 0) with budget left
-        const uint32_t keep_t = E == 0 ? (last1 ? 1u : 0x3FFu) : 0u;
+        const uint32_t keep_t = e0 ? (last1 ? 1u : 0x3FFu) : 0u;
         uint32_t pbits = vbits & (~tbits | keep_t);
-        uint32_t cbits = last1 ? (pbits & 0x3FEu) : 0u;
-        const uint32_t cshift = strand ? 10u : 20u;      // packed counters: branch (bits 0-9) | chain strand 1 (10-19) | strand 0 (20-29)
+        uint32_t cbits = pbits & ((run_b ? 0x21Eu : 0u) | (run_d ? 0x1E0u : 0u));
+        const uint32_t cshift = strand ? 10u : 20u;      // packed counters: branch (bits 0-9) | run strand 1 (10-19) | strand 0 (20-29)
 
-        // slots: warp scan of (branch pushes | chain pushes << 16); net growth decides who is kept
+        // slots: warp scan of (branch pushes | run pushes << 10/20); net growth decides who is kept
         const uint32_t mine = (uint32_t)__popc(pbits & ~cbits) | ((uint32_t)__popc(cbits) << cshift);
         uint32_t incl = mine;
 #pragma unroll
@@ -432,20 +516,17 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
             if ((int)lane >= o) incl += v;
         }
-        // lanes 0..lane kept, the lanes behind un-popped: ring and chain occupancy after the step
+        // lanes 0..lane kept, the lanes behind un-popped: ring and run-stack occupancy after the step
         const uint32_t ring_if = bcnt - (lane + 1u) + (incl & 1023u);
         const uint32_t chain_if = c0 + c1 + ((incl >> 10) & 1023u) + (incl >> 20);
-        const bool fits = act && ring_if + R <= BCAP && chain_if <= CCAP;
+        const bool fits = act && ring_if <= BCAP && chain_if <= CCAP;
         uint32_t keepmask = __ballot_sync(0xffffffffu, fits);
         uint32_t akeep = keepmask == 0xffffffffu ? 32u : (uint32_t)(__ffs(~keepmask) - 1);   // leading run
         if (akeep > a) akeep = a;
-        if (akeep == 0) {                                 // lane 0 alone may use the whole ring
-            const uint32_t r0 = __shfl_sync(0xffffffffu, ring_if, 0), c0 = __shfl_sync(0xffffffffu, chain_if, 0);
-            if (r0 <= BCAP && c0 <= CCAP) akeep = 1;
-        }
-        if (akeep == 0) {
-            if (c0 + c1 == 0) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // cannot happen (pool bound)
-            force_drain = true;                           // nothing popped; make room first
+        if (akeep == 0) {                                 // not even lane 0 fits
+            const uint32_t ch0 = __shfl_sync(0xffffffffu, chain_if, 0);
+            if (ch0 <= CCAP) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 4ull); break; }   // ring full and nowhere to spill
+            force_drain = true;                           // nothing popped; make room on the run stacks first
             n_cancel += a;
             continue;
         }
@@ -463,26 +544,26 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         n_xsect += (act && straddle) ? 1u : 0u;
 
         if (pbits) {
-            if (pbits & 1u) {
+            if (pbits & 1u) {                             // the match child stays a branch state (same d, same bounds)
                 ent_store(P, (bpos++) & BM, qid, sel4(nk[0], nk[1], nk[2], nk[3], qb), sel4(ns[0], ns[1], ns[2], ns[3], qb),
                           sel4(nk2[0], nk2[1], nk2[2], nk2[3], qb), ma_lo, ma_hi);
             }
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 if (pbits & (2u << b)) {
-                    if (last1) { ent_store(Cq, cpos, qid, nk[b], ns[b], nk2[b], ma_lo | cb1, mm_hi); cpos += cstep; }
+                    if (run_b) { ent_store(Cq, cpos, qid, nk[b], ns[b], nk2[b], ma_lo | cb1, mm_hi); cpos += cstep; }
                     else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], ma_lo, mm_hi);
                 }
             }
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 if (pbits & (32u << b)) {
-                    if (last1) { ent_store(Cq, cpos, qid, nk[b], ns[b], nk2[b], de_lo | cb0, de_hi); cpos += cstep; }
+                    if (run_d) { ent_store(Cq, cpos, qid, nk[b], ns[b], nk2[b], de_lo | cb0, de_hi); cpos += cstep; }
                     else ent_store(P, (bpos++) & BM, qid, nk[b], ns[b], nk2[b], de_lo, de_hi);
                 }
             }
             if (pbits & 512u) {
-                if (last1) { ent_store(Cq, cpos, qid, k, s, k2, in_lo | cb1, mm_hi); cpos += cstep; }
+                if (run_b) { ent_store(Cq, cpos, qid, k, s, k2, in_lo | cb1, mm_hi); cpos += cstep; }
                 else ent_store(P, (bpos++) & BM, qid, k, s, k2, in_lo, mm_hi);
             }
         }
@@ -502,7 +583,18 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         __syncwarp();
     }
     flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
-    if (lane == 0) atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
+    if (lane == 0) {
+        atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
+        atomicMax(&ctr[BC_CTR_SPILLMAX], (unsigned long long)gsp_max);
+    }
+}
+
+template <bool SMALL, bool HAS_N>
+cudaError_t launch_search(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
+    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    bc_search_kernel<SMALL, HAS_N><<<grid, threads, smem, st>>>(p);
+    return cudaGetLastError();
 }
 
 }  // namespace
@@ -510,9 +602,9 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 cudaError_t bc_launch_search(const BcSearchParams &p, int sm_count, uint32_t ctas_per_sm, uint32_t warps_per_cta,
                              cudaStream_t st) {
     if (p.ws.nq == 0) return cudaSuccess;
-    size_t smem = (size_t)warps_per_cta * (p.bcap + p.ccap) * BC_POOL_ENTRY_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    bc_search_kernel<<<sm_count * ctas_per_sm, warps_per_cta * 32, smem, st>>>(p);
-    return cudaGetLastError();
+    const size_t smem = (size_t)warps_per_cta * (p.bcap + p.ccap) * BC_POOL_ENTRY_BYTES;
+    const int grid = sm_count * (int)ctas_per_sm, threads = (int)warps_per_cta * 32;
+    const bool small = p.o.z <= BC_QREC_SMALL_Z && p.o.seed_z <= BC_QREC_SMALL_SZ, has_n = p.ws.q_noff != 0;
+    if (small) return has_n ? launch_search<true, true>(p, grid, threads, smem, st) : launch_search<true, false>(p, grid, threads, smem, st);
+    return has_n ? launch_search<false, true>(p, grid, threads, smem, st) : launch_search<false, false>(p, grid, threads, smem, st);
 }

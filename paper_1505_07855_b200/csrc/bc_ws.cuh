@@ -3,13 +3,21 @@
 #pragma once
 #include "bc_internal.cuh"
 
-// prepared query entry (uint16) for consumption step t of query q = 2*read + strand:
-//   bits 0-2  base consumed at step t (strand 1: complemented), 4 = N
-//   bits 3-8  D[t]  = lower bound on differences needed for W[t..m-1], clamped to 63
-//   bits 9-14 Ds[t] = same for the unconsumed seed part W[t..seed_len-1] (0 outside the seed)
-#define BC_PREP_BASE(p) ((p) & 7u)
-#define BC_PREP_D(p) (((p) >> 3) & 63u)
-#define BC_PREP_DS(p) (((p) >> 9) & 63u)
+// Prepared query RECORD (one per query q = 2*read + strand, `qstride` bytes, 16-byte aligned), written by
+// bc_prepare_kernel and read by the search kernel -- everything a search node needs to know about its
+// query, compact enough to stay cache-resident beside an index far larger than L2:
+//   [0 .. q_soff)        thrD[r], r = 0..z   (bytes): smallest t with D[t] <= r, clamped to 255
+//   [q_soff .. q_boff)   thrS[r], r = 0..seed_z      : the same for Ds[] (0 when the seed is off)
+//   [q_boff .. q_noff)   the query's bases, 2 bits each, base t at bits 2*(t%16) of word t/16
+//                        (strand 1: already complemented), max_len/16 + 1 words
+//   [q_noff .. qstride)  1 bit per base: N (only when the batch carries an N mask)
+// D[t] = lower bound on the differences W[t..m-1] needs, Ds[t] the same for the unconsumed
+// seed part; both never increase with t, so a budget check "D[t] <= r" is "t >= thrD[r]".  A threshold
+// that is rounded DOWN (the clamp, m = 256 only) weakens the prune, never the result.
+// Small budgets (z <= 7, seed_z <= 3): thrD in bytes 0-7, thrS in bytes 8-11, q_boff = 16, so that one
+// 128-bit load brings every threshold into registers (BC_QREC_SMALL).
+#define BC_QREC_SMALL_Z 7
+#define BC_QREC_SMALL_SZ 3
 
 enum {                      // indices into the uint64 counter block
     BC_CTR_TICKET = 0,      // next query to hand to a warp
@@ -17,7 +25,7 @@ enum {                      // indices into the uint64 counter block
     BC_CTR_NODES = 2,
     BC_CTR_LOOKUPS = 3,
     BC_CTR_LINES = 4,
-    BC_CTR_ERROR = 5,       // bit 0: bad read length, bit 1: pool overflow (must never happen)
+    BC_CTR_ERROR = 5,       // bit 0: bad read length, bit 1: pool overflow (must never happen), bit 2: spill area exhausted
     BC_CTR_DLOOKUPS = 6,
     BC_CTR_POOLMAX = 7,
     BC_CTR_NBIG = 8,        // queries whose raw segment is sorted by a whole CTA
@@ -27,14 +35,15 @@ enum {                      // indices into the uint64 counter block
     BC_CTR_CSTEPS = 12,     // warp-level chain iterations
     BC_CTR_CANCEL = 13,     // branch states popped and put back because their children did not fit
     BC_CTR_SPILL = 14,      // 32-entry blocks moved from the branch rings to global memory
+    BC_CTR_SPILLMAX = 15,   // deepest per-warp spill stack seen (blocks)
     BC_CTR_COUNT = 16
 };
 
 struct BcRawHit { uint32_t qid, k, l, d; };
 
 struct BcWorkspace {        // device pointers into the caller's workspace
-    uint16_t *prep;         // [nq][stride]
-    uint32_t stride;
+    uint8_t *qrec;          // [nq][qstride] prepared query records (layout above)
+    uint32_t qstride, q_soff, q_boff, q_noff;
     uint32_t *qcnt;         // [nq] raw hits per query
     uint32_t *qfill;        // [nq] scatter cursors, later: unique hits per query
     uint64_t *seg_off;      // [nq+1] exclusive scan of qcnt

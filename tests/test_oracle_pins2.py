@@ -232,3 +232,24 @@ def test_seed_limit_equals_filter_of_unseeded_alignments_gaps_off():
         assert have == want
         checked += len(want)
     assert checked >= 30
+
+
+# ------------------------------------------------------------------------------- C8: the bucketed suffix sort
+@pytest.mark.parametrize("n,alpha", [(1, 4), (5, 1), (11, 2), (12, 4), (13, 4), (300, 1), (5000, 2), (200_000, 4)])
+def test_c8_bucketed_suffix_sort_equals_literal_sort(n, alpha):
+    """SURVEY C8 allows bucketing by the first 12 bases at sizes the literal sort cannot reach; both builds must
+    give the same index (SA, BWT, C, primary) -- incl. texts shorter than the bucket key, runs of one base
+    (every suffix in bucket 0 or padded into it) and suffixes that end inside the key."""
+    rng = np.random.default_rng(n * 7 + alpha)
+    T = rng.integers(0, alpha, size=n).astype(np.uint8)
+    if n >= 5000:
+        T[100:160] = T[1000:1060]                 # a repeat: deep comparisons inside one bucket
+        T[-40:] = 0                               # a run of A at the end: suffixes that are all padding
+    a, b = Oracle(T, nthreads=3, sort="literal"), Oracle(T, nthreads=3, sort="bucketed")
+    for which in (0, 1):
+        SA_a, B_a, C_a, p_a = a.index(which)
+        SA_b, B_b, C_b, p_b = b.index(which)
+        assert np.array_equal(SA_a, SA_b) and np.array_equal(B_a, B_b) and np.array_equal(C_a, C_b) and p_a == p_b
+    if n <= 300:
+        from tests.bruteforce import suffix_rows
+        assert b.index(0)[0].tolist() == suffix_rows(T.tolist())
