@@ -183,9 +183,11 @@ int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
 /* More tuning (0 = default): spill_blocks = per-warp spill area of the branch rings in blocks of 32
  * states (default 128; bc_align_batch returns BC_E_NOMEM when a warp's area runs full -- raise it, ask
  * bc_align_workspace_bytes again and repeat the call); pool_kb = shared memory per SM given to the
- * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond).  Affects the
- * workspace size: set it before bc_align_workspace_bytes. */
-int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb);
+ * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond); ld_policy = cache
+ * policy of the index loads, 1 = default, 2 = no L1 allocation + 64-byte L2 prefetch size (default: 1 for
+ * an index up to 64 MB, 2 beyond).  spill_blocks affects the workspace size: set it before
+ * bc_align_workspace_bytes. */
+int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb, uint32_t ld_policy);
 
 /* Host-side index construction for synthetic genomes (untimed helper): suffix sort
  * of T$ and reverse(T)$ -> transport arrays.  text: HOST, n codes 0..3.  The arrays are allocated

@@ -67,13 +67,21 @@ class BcError(RuntimeError):
 
 
 _lib = None
+_lib_path = None
+
+
+def use_library(path: str | None):
+    """Load a build-time variant of the library (see _build.build_variant) instead of the default one; None =
+    back to the default.  Handles created by one library must not be passed to another: call this first."""
+    global _lib, _lib_path
+    _lib, _lib_path = None, path
 
 
 def lib():
     """The loaded C-ABI library.  Built in-tree with nvcc if missing or stale; raises otherwise."""
     global _lib
     if _lib is None:
-        so = _build.build()
+        so = _lib_path or os.environ.get("BC_LIBRARY") or _build.build()
         if not os.path.exists(so):
             raise ImportError("libbarracuda_b200.so is missing and could not be built; there is no CPU fallback")
         L = C.CDLL(so)
@@ -92,7 +100,7 @@ def lib():
         L.bc_locate.argtypes = [vp, vp, u64, vp, vp]
         L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 16)]
         L.bc_set_geometry.argtypes = [vp, u32, u32]
-        L.bc_set_tuning.argtypes = [vp, u32, u32]
+        L.bc_set_tuning.argtypes = [vp, u32, u32, u32]
         L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
         L.bc_index_build_gpu_bytes.argtypes = [u64, u32, u32, C.POINTER(C.c_size_t)]
@@ -167,21 +175,20 @@ class HostIndex:
         cnt = self.n // s.sa_interval + 1
         return np.ctypeslib.as_array(C.cast(s.sa, C.POINTER(C.c_uint32)), shape=(cnt,)), int(s.sa_interval)
 
-    def save(self, path: str):
-        """Cache the transport arrays on disk (config 5: "index built once on the host and cached")."""
+    def to_arrays(self) -> dict:
+        """The transport arrays as a dict of numpy arrays (views; copy before the index is freed)."""
         st = self.struct
         d = {"n": np.uint64(self.n), "sa_interval": np.uint32(st.sa_interval), "sa": self.sa_samples()[0]}
         for name, which in (("fwd", 0), ("rev", 1)):
             bwt2, occ, Cc, primary, oi = self.arrays(which)
             d[name + "_bwt2"], d[name + "_occ"] = bwt2, occ
             d[name + "_C"], d[name + "_primary"], d[name + "_oi"] = np.asarray(Cc, np.uint64), np.uint64(primary), np.uint32(oi)
-        np.savez(path, **d)
+        return d
 
     @staticmethod
-    def load(path: str) -> "HostIndex":
-        """A bc_index_host over numpy arrays read back from save(); Python owns the memory."""
-        z = np.load(path)
-        keep = {k: np.ascontiguousarray(z[k]) for k in z.files}
+    def from_arrays(arrs: dict) -> "HostIndex":
+        """A bc_index_host over numpy arrays (to_arrays() of another process, or a file); Python owns the memory."""
+        keep = {k: np.ascontiguousarray(v) for k, v in arrs.items()}
         h = bc_index_host()
         for name, b in (("fwd", h.fwd), ("rev", h.rev)):
             b.n = int(keep["n"]); b.primary = int(keep[name + "_primary"]); b.occ_interval = int(keep[name + "_oi"])
@@ -192,6 +199,15 @@ class HostIndex:
         obj = HostIndex(C.pointer(h))
         obj._owned, obj._keep = False, (keep, h)
         return obj
+
+    def save(self, path: str):
+        """Cache the transport arrays on disk (config 5: "index built once on the host and cached")."""
+        np.savez(path, **self.to_arrays())
+
+    @staticmethod
+    def load(path: str) -> "HostIndex":
+        z = np.load(path)
+        return HostIndex.from_arrays({k: z[k] for k in z.files})
 
     def free(self):
         if self._p is not None:
@@ -225,7 +241,7 @@ class DeviceIndex:
 
     def __init__(self, handle, mem, n, device):
         self._h, self.mem, self.n, self.device = handle, mem, n, device
-        self.spill_blocks, self.pool_kb = 0, 0
+        self.spill_blocks, self.pool_kb, self.ld_policy = 0, 0, 0
 
     @property
     def handle(self):
@@ -270,9 +286,9 @@ def bc_set_geometry(ix: DeviceIndex, ctas_per_sm: int = 0, warps_per_cta: int = 
     _check(lib().bc_set_geometry(ix.handle, ctas_per_sm, warps_per_cta), "bc_set_geometry")
 
 
-def bc_set_tuning(ix: DeviceIndex, spill_blocks: int = 0, pool_kb: int = 0):
-    _check(lib().bc_set_tuning(ix.handle, spill_blocks, pool_kb), "bc_set_tuning")
-    ix.spill_blocks, ix.pool_kb = spill_blocks, pool_kb
+def bc_set_tuning(ix: DeviceIndex, spill_blocks: int = 0, pool_kb: int = 0, ld_policy: int = 0):
+    _check(lib().bc_set_tuning(ix.handle, spill_blocks, pool_kb, ld_policy), "bc_set_tuning")
+    ix.spill_blocks, ix.pool_kb, ix.ld_policy = spill_blocks, pool_kb, ld_policy
 
 
 STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry",
@@ -406,7 +422,7 @@ def bc_align_batch(ix: DeviceIndex, reads: DeviceReads, opts, ws: Workspace | No
             return AlignResult(ws.hit_offsets, ws.hits, int(need[0]), int(need[1])), ws
         if rc == BC_E_NOMEM and grow and (ix.spill_blocks or 128) < 8192:
             # a warp's spill area of pending branch states ran full: give it more and repeat (never truncated)
-            bc_set_tuning(ix, 4 * (ix.spill_blocks or 128), ix.pool_kb)
+            bc_set_tuning(ix, 4 * (ix.spill_blocks or 128), ix.pool_kb, ix.ld_policy)
             ws = Workspace(ix, reads.n_reads, max(1, reads.max_len), opts, ws.raw_hits_per_read, ws.hits_capacity)
             continue
         if rc != BC_E_OVERFLOW or not grow:

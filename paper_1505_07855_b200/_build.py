@@ -30,6 +30,24 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def build_variant(defines: dict, force: bool = False) -> str:
+    """A build-time VARIANT of the library (autotuner): the same sources compiled with
+    -DNAME=VALUE for every item of `defines`, as paper_1505_07855_b200/variants/libbarracuda_b200_<tag>.so."""
+    tag = "_".join(f"{k.lower().replace('bc_', '')}{v}" for k, v in sorted(defines.items())) or "default"
+    out_dir = os.path.join(_DIR, "variants")
+    os.makedirs(out_dir, exist_ok=True)
+    so = os.path.join(out_dir, f"libbarracuda_b200_{tag}.so")
+    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS]
+    if not force and os.path.exists(so) and all(os.path.getmtime(d) <= os.path.getmtime(so) for d in deps):
+        return so
+    cmd = [_nvcc()] + NVCC_FLAGS + [f"-D{k}={v}" for k, v in sorted(defines.items())] + ["-o", so] + \
+          [os.path.join(CSRC, s) for s in SOURCES]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + r.stdout + r.stderr)
+    return so
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every CUDA source of the library for sm_100a into one shared object."""
     if not force and not stale():

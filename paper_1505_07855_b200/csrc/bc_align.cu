@@ -157,6 +157,7 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     const uint32_t ctas = g.ctas, warps = g.warps;
     p.bcap = g.bcap;
     p.ccap = g.ccap;
+    p.ld_policy = ix->ld_policy ? ix->ld_policy - 1u : (ix->bytes > ((size_t)64 << 20) ? 1u : 0u);
     ws.spill = (uint2 *)(base + L.off_spill);
     ws.spill_blocks = L.spill_blocks;
 

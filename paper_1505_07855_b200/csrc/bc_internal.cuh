@@ -45,6 +45,7 @@ struct bc_index {            // the opaque handle of the ABI
     uint32_t ctas_per_sm, warps_per_cta;   // 0 = chosen by the library (bc_set_geometry)
     uint32_t spill_blocks;   // per-warp spill area of the branch rings, blocks of 32 states (bc_set_tuning)
     uint32_t pool_kb;        // shared memory per SM given to the state pools, 0 = by index size (bc_set_tuning)
+    uint32_t ld_policy;      // cache policy of the index loads: 0 = by index size, 1 = default, 2 = no L1 / 64 B L2
     uint64_t stats[16];
     int sm_count;
     cudaEvent_t ev[2];       // around the search kernel of the last bc_align_batch (stats[6])
@@ -60,14 +61,24 @@ __device__ __forceinline__ uint32_t bc_rank_pos(const BcBwtDev &b, uint32_t x) {
 
 struct BcBlockRegs { uint32_t c0, c1, c2, c3; uint64_t lo, hi; };
 
+// The one load that carries the whole search, with two cache policies (chosen per index size by the host,
+// bc_set_tuning; measured on the 1 Gbp index: L1 hit rate of index sectors 9 %, +5 % reads/s with policy 1):
+//   LD = 0  read-only path, default policies          (index resident in L2: L1 helps the top of the trees)
+//   LD = 1  read-only path, no L1 allocation, 64-byte L2 prefetch size (index far beyond L2)
 // one 256-bit read-only load of the block that holds position p of the '$'-less string
+template <int LD = 0>
 __device__ __forceinline__ BcBlockRegs bc_load_block(const uint4 *lines, uint32_t p) {
     const uint4 *q = lines + (size_t)(p >> 6) * 2;
     BcBlockRegs r;
     uint32_t l0, l1, h0, h1;
-    asm("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-        : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
-        : "l"(q));
+    if (LD == 1)
+        asm("ld.global.nc.L1::no_allocate.L2::64B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
+            : "l"(q));
+    else
+        asm("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
+            : "l"(q));
     r.lo = ((uint64_t)l1 << 32) | l0;
     r.hi = ((uint64_t)h1 << 32) | h0;
     return r;
@@ -86,8 +97,9 @@ __device__ __forceinline__ void bc_block_rank4(const BcBlockRegs &r, uint32_t p,
 }
 
 // all four O(., .) before position p of the '$'-less string
+template <int LD = 0>
 __device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_t out[4]) {
-    bc_block_rank4(bc_load_block(lines, p), p, out);
+    bc_block_rank4(bc_load_block<LD>(lines, p), p, out);
 }
 
 // one symbol's count from a loaded block: #{j < p : B'[j] = c}  (c > 3 gives a don't-care value)

@@ -219,7 +219,7 @@ __device__ __forceinline__ uint32_t run_end(const QThr &q, int dc, int sdc, int 
 // Stack layout inside the run area Cq[0..CCAP): strand 1 grows up from 0, strand 0 down from CCAP-1.
 // The caller guarantees 32 free ring slots per iteration (the loop re-checks).
 // ---------------------------------------------------------------------------------------------
-template <bool S0, bool HAS_N>
+template <bool S0, bool HAS_N, int LD>
 __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4 *lines, uint32_t primary,
                                             const uint32_t *Cs, uint2 *Cq, uint32_t CCAP, uint32_t &cnt,
                                             bool drain, uint2 *P, uint32_t bb, uint32_t &bcnt, uint32_t BCAP,
@@ -245,7 +245,7 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             const bool two = (plo >> 6) != (phi >> 6);
-            const BcBlockRegs rlo = bc_load_block(lines, plo);
+            const BcBlockRegs rlo = bc_load_block<LD>(lines, plo);
             n_xsect += two ? 1u : 0u;
             // strand 0 also needs one OTHER symbol's count for the forward start k2 (see below):
             // x = A when c is A or C, x = T when c is G or T
@@ -253,7 +253,7 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
             uint32_t olo = bc_block_rank1(rlo, plo, c), ohi, xlo = 0, xhi = 0;
             if (S0) xlo = bc_block_rank1(rlo, plo, x);
             if (two) {                                    // most narrow intervals sit in one sector
-                const BcBlockRegs rhi = bc_load_block(lines, phi);
+                const BcBlockRegs rhi = bc_load_block<LD>(lines, phi);
                 ohi = bc_block_rank1(rhi, phi, c);
                 if (S0) xhi = bc_block_rank1(rhi, phi, x);
             } else {
@@ -310,7 +310,7 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
 // free and comes back when the ring runs low; if that area is ever full the warp raises error bit 2
 // (BC_E_NOMEM: the caller passes a larger spill area), never a silent truncation.
 // ---------------------------------------------------------------------------------------------
-template <bool SMALL, bool HAS_N>
+template <bool SMALL, bool HAS_N, int LD>
 __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
@@ -407,8 +407,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         if (c1 >= 32u || c0 >= 32u || ((bcnt == 0 || force_drain) && c0 + c1 > 0u)) {
             if (bcnt + 32u > BCAP) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 4ull); break; }   // spill area exhausted
             const bool drain = bcnt == 0 || force_drain;
-            chain_steps<false, HAS_N>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
-            chain_steps<true, HAS_N>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
+            chain_steps<false, HAS_N, LD>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
+            chain_steps<true, HAS_N, LD>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
             force_drain = false;
             continue;
         }
@@ -446,8 +446,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             uint32_t olo[4], ohi[4];
-            bc_rank4(lines, plo, olo);                    // two unconditional loads: predicating the second one on
-            bc_rank4(lines, phi, ohi);                    // "other sector" was measured 3 % slower here (not in the run step)
+            bc_rank4<LD>(lines, plo, olo);                   // two unconditional loads: predicating the second one on
+            bc_rank4<LD>(lines, phi, ohi);                   // "other sector" was measured 3 % slower here (not in the run step)
             straddle = (plo >> 6) != (phi >> 6);
             const uint4 Cv = *reinterpret_cast<const uint4 *>(Ctab + strand * 4u);
             const uint32_t Cc[4] = {Cv.x, Cv.y, Cv.z, Cv.w};
@@ -589,12 +589,17 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     }
 }
 
-template <bool SMALL, bool HAS_N>
+template <bool SMALL, bool HAS_N, int LD>
 cudaError_t launch_search(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    bc_search_kernel<SMALL, HAS_N><<<grid, threads, smem, st>>>(p);
+    bc_search_kernel<SMALL, HAS_N, LD><<<grid, threads, smem, st>>>(p);
     return cudaGetLastError();
+}
+
+template <bool SMALL, bool HAS_N>
+cudaError_t launch_search_ld(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
+    return p.ld_policy ? launch_search<SMALL, HAS_N, 1>(p, grid, threads, smem, st) : launch_search<SMALL, HAS_N, 0>(p, grid, threads, smem, st);
 }
 
 }  // namespace
@@ -605,6 +610,6 @@ cudaError_t bc_launch_search(const BcSearchParams &p, int sm_count, uint32_t cta
     const size_t smem = (size_t)warps_per_cta * (p.bcap + p.ccap) * BC_POOL_ENTRY_BYTES;
     const int grid = sm_count * (int)ctas_per_sm, threads = (int)warps_per_cta * 32;
     const bool small = p.o.z <= BC_QREC_SMALL_Z && p.o.seed_z <= BC_QREC_SMALL_SZ, has_n = p.ws.q_noff != 0;
-    if (small) return has_n ? launch_search<true, true>(p, grid, threads, smem, st) : launch_search<true, false>(p, grid, threads, smem, st);
-    return has_n ? launch_search<false, true>(p, grid, threads, smem, st) : launch_search<false, false>(p, grid, threads, smem, st);
+    if (small) return has_n ? launch_search_ld<true, true>(p, grid, threads, smem, st) : launch_search_ld<true, false>(p, grid, threads, smem, st);
+    return has_n ? launch_search_ld<false, true>(p, grid, threads, smem, st) : launch_search_ld<false, false>(p, grid, threads, smem, st);
 }

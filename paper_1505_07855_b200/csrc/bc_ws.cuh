@@ -66,7 +66,8 @@ struct BcSearchParams {
     bc_opts o;
     BcWorkspace ws;
     uint32_t bcap;          // branch ring entries per warp (power of two)
-    uint32_t ccap;          // chain stack entries per warp
+    uint32_t ccap;          // run stack entries per warp (both strands)
+    uint32_t ld_policy;     // 0 = default cache policies for the index loads, 1 = no L1 allocation + 64 B L2 prefetch size
 };
 
 // launchers (return cudaError_t of the launch)

@@ -58,6 +58,43 @@ def max_over_ranks(x: float, device=None) -> float:
     return float(t.item())
 
 
+def broadcast_array(a, device=None, src: int = 0):
+    """numpy array of rank `src` on every rank (other ranks pass None).  Shape and dtype travel first."""
+    if not active():
+        return a
+    import torch
+    d = _dist()
+    meta = [(a.shape, a.dtype.str) if d.get_rank() == src else None]
+    d.broadcast_object_list(meta, src=src)
+    shape, dt = meta[0]
+    on_gpu = d.get_backend() == "nccl"
+    if d.get_rank() == src:
+        t = torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1))
+    else:
+        t = torch.empty(int(np.prod(shape, dtype=np.int64)) * np.dtype(dt).itemsize, dtype=torch.uint8)
+    if on_gpu:
+        t = t.to(device)
+    if t.numel():
+        d.broadcast(t, src=src)
+    out = t.cpu().numpy().view(np.dtype(dt)).reshape(shape)
+    return a if d.get_rank() == src else out
+
+
+def broadcast_host_index(host, device=None, src: int = 0):
+    """The index is built ONCE (rank `src`) and its transport arrays are shipped to the other ranks -- one suffix
+    sort instead of one per GPU ("one broadcast over NVLink at upload").  Returns a HostIndex everywhere."""
+    if not active():
+        return host
+    from . import HostIndex
+    d = _dist()
+    names = ["n", "sa_interval", "sa"] + [p + s for p in ("fwd", "rev") for s in ("_bwt2", "_occ", "_C", "_primary", "_oi")]
+    arrs = host.to_arrays() if d.get_rank() == src else {}
+    out = {}
+    for nm in names:
+        out[nm] = broadcast_array(np.asarray(arrs[nm]) if d.get_rank() == src else None, device, src)
+    return host if d.get_rank() == src else HostIndex.from_arrays(out)
+
+
 def gather_csr(hit_offsets: np.ndarray, hits: np.ndarray):
     """Concatenate per-rank CSR results in rank order on rank 0 (offsets rebased); other ranks get
     None.  Host-side, after the timed region."""

@@ -65,3 +65,42 @@ def test_two_rank_sharding_matches_single_rank():
     T = sd.make_genome(cfg)
     off1, hits1 = Oracle(T, nthreads=2).align(sd.make_reads(cfg, T).codes, cfg.opts.astuple())
     assert np.array_equal(off, off1) and hits.tobytes() == hits1.tobytes()
+
+
+def _bcast_worker(rank, world, port, q):
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import paper_1505_07855_b200 as bc
+    bdist.init_from_env("gloo")
+    cfg = sd.CONFIGS["2"].scaled(n=30_000)
+    host = genome = None
+    if rank == 0:                                    # the index is built once, on rank 0 only
+        genome = sd.make_genome(cfg)
+        host = bc.bc_index_build_host(genome, 128, 32, 2)
+    genome = bdist.broadcast_array(genome)
+    host = bdist.broadcast_host_index(host)
+    a = host.to_arrays()
+    q.put((rank, genome.tobytes(), {k: np.asarray(v).tobytes() for k, v in a.items()}))
+    bdist.barrier()
+    bdist.finish()
+
+
+def test_index_built_once_and_broadcast():
+    """rank 0 builds the index; the other rank receives the genome and every transport array bit for bit."""
+    ctx = mp.get_context("spawn")
+    q = ctx.SimpleQueue()
+    port = _free_port()
+    procs = [ctx.Process(target=_bcast_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict()
+    for _ in range(2):
+        r, g, arrs = q.get()
+        got[r] = (g, arrs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert got[0][0] == got[1][0] and len(got[0][0]) == 30_000
+    assert got[0][1].keys() == got[1][1].keys() and len(got[0][1]) == 13
+    for k in got[0][1]:
+        assert got[0][1][k] == got[1][1][k], k
