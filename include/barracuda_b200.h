@@ -174,7 +174,8 @@ int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint3
  * [9] nodes expanded in branch steps, [10] warp-level chain iterations, [11] nodes expanded in
  * chain iterations, [12] branch states popped and put back because their children did not fit,
  * [13] 32-entry blocks of branch states spilled from the on-chip rings to the workspace,
- * [14] deepest per-warp spill stack seen (blocks), [15] passes (best-stratum mode). */
+ * [14] deepest per-warp spill stack seen (blocks), [15] bc_align_batch: blocks of 32 pending states that moved
+ * from a busy warp to an idle one; bc_align_batch_best: largest per-read budget searched + 1. */
 int bc_last_stats(const bc_index *ix, uint64_t *out16);
 
 /* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM (<= 8), warps per CTA (<= 8). */
@@ -185,8 +186,8 @@ int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
  * bc_align_workspace_bytes again and repeat the call); pool_kb = shared memory per SM given to the
  * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond); ld_policy = cache
  * policy of the index loads, 1 = default, 2 = no L1 allocation + 64-byte L2 prefetch size (default: 1 for
- * an index up to 64 MB, 2 beyond).  spill_blocks affects the workspace size: set it before
- * bc_align_workspace_bytes. */
+ * an index up to 64 MB, 2 beyond); ld_policy + 256 switches the exchange of pending states between warps
+ * off (A/B measurements).  spill_blocks affects the workspace size: set it before bc_align_workspace_bytes. */
 int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb, uint32_t ld_policy);
 
 /* Host-side index construction for synthetic genomes (untimed helper): suffix sort

@@ -189,13 +189,16 @@ class HostIndex:
     def from_arrays(arrs: dict) -> "HostIndex":
         """A bc_index_host over numpy arrays (to_arrays() of another process, or a file); Python owns the memory."""
         keep = {k: np.ascontiguousarray(v) for k, v in arrs.items()}
+
+        def scalar(name):
+            return int(keep[name].reshape(-1)[0])
         h = bc_index_host()
         for name, b in (("fwd", h.fwd), ("rev", h.rev)):
-            b.n = int(keep["n"]); b.primary = int(keep[name + "_primary"]); b.occ_interval = int(keep[name + "_oi"])
+            b.n = scalar("n"); b.primary = scalar(name + "_primary"); b.occ_interval = scalar(name + "_oi")
             b.bwt2 = keep[name + "_bwt2"].ctypes.data; b.occ = keep[name + "_occ"].ctypes.data
             for c in range(5):
-                b.C[c] = int(keep[name + "_C"][c])
-        h.sa_interval = int(keep["sa_interval"]); h.sa = keep["sa"].ctypes.data
+                b.C[c] = int(keep[name + "_C"].reshape(-1)[c])
+        h.sa_interval = scalar("sa_interval"); h.sa = keep["sa"].ctypes.data
         obj = HostIndex(C.pointer(h))
         obj._owned, obj._keep = False, (keep, h)
         return obj
@@ -292,7 +295,7 @@ def bc_set_tuning(ix: DeviceIndex, spill_blocks: int = 0, pool_kb: int = 0, ld_p
 
 
 STAT_NAMES = ("nodes", "lookups", "lines", "raw_hits", "d_lookups", "pool_max", "search_ns", "geometry",
-              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes", "cancelled", "spill_blocks", "spill_max", "passes")
+              "branch_steps", "branch_nodes", "chain_steps", "chain_nodes", "cancelled", "spill_blocks", "spill_max", "passes_or_steals")
 
 
 def bc_last_stats(ix: DeviceIndex) -> dict:
@@ -515,11 +518,15 @@ def bc_align_batch_best(ix: DeviceIndex, reads: DeviceReads, opts, stratum_plus:
     caller-owned buffers and repeats on BC_E_OVERFLOW.  Returns (AlignResult, BestWorkspace)."""
     if ws is None:
         ws = BestWorkspace(ix, reads.n_reads, max(1, reads.max_len), opts)
-    for _ in range(5):
+    for _ in range(8):
         rc = bc_align_batch_best_raw(ix, reads, opts, stratum_plus, ws, stream)
         need = ws.needed.cpu().numpy().view(np.uint64)
         if rc == BC_OK:
             return AlignResult(ws.hit_offsets, ws.hits, int(need[0]), int(need[1])), ws
+        if rc == BC_E_NOMEM and (ix.spill_blocks or 128) < 8192:     # spill area exhausted: more of it, repeat
+            bc_set_tuning(ix, 4 * (ix.spill_blocks or 128), ix.pool_kb, ix.ld_policy)
+            ws = BestWorkspace(ix, reads.n_reads, max(1, reads.max_len), opts, ws.raw_hits_per_read, ws.hits_capacity)
+            continue
         if rc != BC_E_OVERFLOW:
             raise BcError(rc, "bc_align_batch_best")
         per_read = max(2 * ws.raw_hits_per_read, -(-int(need[1]) // max(1, reads.n_reads)) + 1)

@@ -11,7 +11,7 @@ constexpr uint64_t SCAN_TILE = 256 * 8;            // must match bc_post.cu
 constexpr size_t RAW_BYTES = sizeof(BcRawHit) + sizeof(uint64_t) + sizeof(uint32_t);   // arena + seg_key + seg_d
 
 struct WsLayout {
-    size_t off_qrec, off_spill, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_ctr, fixed;
+    size_t off_qrec, off_qz, off_spill, off_qcnt, off_qfill, off_seg_off, off_uoff, off_blk, off_big, off_sqf, off_ctr, off_sqb, fixed;
     uint32_t qstride, q_soff, q_boff, q_noff, nq, spill_blocks;
 };
 
@@ -37,6 +37,7 @@ int make_ws_layout(uint32_t n_reads, uint32_t max_len, const bc_opts *o, bool wi
     qrec_layout(o, max_len, with_n, L);
     size_t x = 0;
     L.off_qrec = x;    x = align_up(x + qrec_bytes, 256);
+    L.off_qz = x;      x = align_up(x + (size_t)n_reads, 256);
     L.off_spill = x;   x = align_up(x + (size_t)grid_warps * spill_blocks * 32 * BC_POOL_ENTRY_BYTES, 256);
     L.off_qcnt = x;    x = align_up(x + (size_t)L.nq * 4, 256);
     L.off_qfill = x;   x = align_up(x + (size_t)L.nq * 4, 256);
@@ -44,7 +45,9 @@ int make_ws_layout(uint32_t n_reads, uint32_t max_len, const bc_opts *o, bool wi
     L.off_uoff = x;    x = align_up(x + ((size_t)L.nq + 1) * 8, 256);
     L.off_blk = x;     x = align_up(x + ((size_t)L.nq / SCAN_TILE + 2) * 8, 256);
     L.off_big = x;     x = align_up(x + (size_t)L.nq * 4, 256);
+    L.off_sqf = x;     x = align_up(x + BC_STEAL_SLOTS * 4, 256);
     L.off_ctr = x;     x = align_up(x + BC_CTR_COUNT * 8, 256);
+    L.off_sqb = x;     x = align_up(x + (size_t)BC_STEAL_SLOTS * 32 * BC_POOL_ENTRY_BYTES, 256);
     L.fixed = x;
     return BC_OK;
 }
@@ -102,8 +105,9 @@ extern "C" int bc_align_workspace_bytes(const bc_index *ix, uint32_t n_reads, ui
     return BC_OK;
 }
 
-extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const bc_opts *o, bc_result *res,
-                              void *d_workspace, size_t ws_bytes, void *cuda_stream) {
+// the hot path; best_plus < 0: exhaustive (bc_align_batch), else the best-stratum mode with that `plus`
+int bc_align_impl(const bc_index *ix_c, const bc_reads *reads, const bc_opts *o, bc_result *res,
+                  void *d_workspace, size_t ws_bytes, void *cuda_stream, int best_plus) {
     bc_index *ix = const_cast<bc_index *>(ix_c);    // statistics live in the handle
     if (!ix || !reads || !res || !d_workspace || ((uintptr_t)d_workspace & 255)) return BC_E_INVAL;
     int rc = check_opts(o);
@@ -136,6 +140,7 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     p.o = *o;
     BcWorkspace &ws = p.ws;
     ws.nq = L.nq;
+    ws.qz = (uint8_t *)(base + L.off_qz);
     ws.qrec = (uint8_t *)(base + L.off_qrec);
     ws.qstride = L.qstride; ws.q_soff = L.q_soff; ws.q_boff = L.q_boff; ws.q_noff = L.q_noff;
     ws.qcnt = (uint32_t *)(base + L.off_qcnt);
@@ -157,11 +162,16 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     const uint32_t ctas = g.ctas, warps = g.warps;
     p.bcap = g.bcap;
     p.ccap = g.ccap;
+    p.best = best_plus >= 0 ? 1u : 0u;
+    p.plus = best_plus >= 0 ? (uint32_t)best_plus : 0u;
     p.ld_policy = ix->ld_policy ? ix->ld_policy - 1u : (ix->bytes > ((size_t)64 << 20) ? 1u : 0u);
     ws.spill = (uint2 *)(base + L.off_spill);
     ws.spill_blocks = L.spill_blocks;
 
-    cudaError_t e = cudaMemsetAsync(base + L.off_qcnt, 0, L.fixed - L.off_qcnt, st);   // qcnt .. ctr
+    ws.sq_flag = (uint32_t *)(base + L.off_sqf);
+    ws.sq_buf = (uint2 *)(base + L.off_sqb);
+    ws.sq_n = ix->no_exchange ? 0u : BC_STEAL_SLOTS;
+    cudaError_t e = cudaMemsetAsync(base + L.off_qcnt, 0, L.off_sqb - L.off_qcnt, st);   // qcnt .. ctr
     if (e == cudaSuccess) e = bc_launch_prepare(p, st);
     if (e == cudaSuccess && ix->ev[0]) e = cudaEventRecord(ix->ev[0], st);
     if (e == cudaSuccess) e = bc_launch_search(p, ix->sm_count, ctas, warps, st);
@@ -189,6 +199,7 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     ix->stats[12] = ctr[BC_CTR_CANCEL];
     ix->stats[13] = ctr[BC_CTR_SPILL];
     ix->stats[14] = ctr[BC_CTR_SPILLMAX];
+    ix->stats[15] = best_plus >= 0 ? ctr[BC_CTR_PASSES] : ctr[BC_CTR_STEALS];
 
     if (ctr[BC_CTR_ERROR] & 1ull) return BC_E_INVAL;        // a read length outside 1..max_len
     if (ctr[BC_CTR_ERROR] & 2ull) return BC_E_CUDA;         // pool discipline violated: a bug, never silent
@@ -197,4 +208,9 @@ extern "C" int bc_align_batch(const bc_index *ix_c, const bc_reads *reads, const
     if (ctr[BC_CTR_ARENA] > cap) return BC_E_OVERFLOW;
     if (ctr[BC_CTR_TOTAL] > res->hits_capacity) return BC_E_OVERFLOW;
     return BC_OK;
+}
+
+extern "C" int bc_align_batch(const bc_index *ix, const bc_reads *reads, const bc_opts *o, bc_result *res,
+                              void *d_workspace, size_t ws_bytes, void *cuda_stream) {
+    return bc_align_impl(ix, reads, o, res, d_workspace, ws_bytes, cuda_stream, -1);
 }

@@ -46,6 +46,7 @@ struct bc_index {            // the opaque handle of the ABI
     uint32_t spill_blocks;   // per-warp spill area of the branch rings, blocks of 32 states (bc_set_tuning)
     uint32_t pool_kb;        // shared memory per SM given to the state pools, 0 = by index size (bc_set_tuning)
     uint32_t ld_policy;      // cache policy of the index loads: 0 = by index size, 1 = default, 2 = no L1 / 64 B L2
+    uint32_t no_exchange;    // 1 = warps keep their states to themselves (bc_set_tuning ld_policy bit 8: A/B measurements)
     uint64_t stats[16];
     int sm_count;
     cudaEvent_t ev[2];       // around the search kernel of the last bc_align_batch (stats[6])

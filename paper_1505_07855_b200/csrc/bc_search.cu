@@ -103,7 +103,8 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 // Pool entry = 24 bytes, array-of-structures, moved with three 64-bit shared-memory accesses:
 //   {qid, k} {s, k2} {mlo, mhi}
 //   mlo = t (bits 0-8) | st (9-10; 0 = M, 1 = I, 2 = D) | n_go (11-18) | n_ge (19-26)
-//   mhi = seed_d (0-7) | d (8-15) | m-1 (16-23)
+//   mhi = seed_d (0-7) | rem (8-15) | m-1 (16-23);  rem = the query's budget - d, the differences still affordable
+//         (the kernel never needs d itself except when a hit is emitted: d = budget - rem)
 //   run entries also carry the base they match next (mlo bits 27-29) and the end of their run - 1 (mhi 24-31)
 // Per warp: a RING of BRANCH states (some difference is affordable at their position), whose cold bottom
 // spills to global memory in blocks of 32, and two stacks of RUN states (see the kernel's comment).
@@ -121,8 +122,10 @@ __device__ __forceinline__ void ent_store(uint2 *P, uint32_t idx, uint32_t qid, 
 }
 
 // warp-aggregated append of raw hits (A5); called by all 32 lanes
+// d = budget - rem: the batch's z, or the read's own current budget in the best-stratum mode (qz != nullptr)
 __device__ __noinline__ void emit_hits(BcRawHit *arena, unsigned long long arena_cap, uint32_t *qcnt,
-                                       unsigned long long *ctr, bool emit, uint32_t qid, uint32_t kf, uint32_t s, uint32_t d) {
+                                       unsigned long long *ctr, bool emit, uint32_t qid, uint32_t kf, uint32_t s, uint32_t rem,
+                                       uint32_t z, const uint8_t *qz) {
     const uint32_t lane = threadIdx.x & 31u;
     uint32_t emask = __ballot_sync(0xffffffffu, emit);
     if (emask == 0) return;
@@ -132,6 +135,7 @@ __device__ __noinline__ void emit_hits(BcRawHit *arena, unsigned long long arena
     base = __shfl_sync(0xffffffffu, base, leader);
     if (emit) {
         unsigned long long pos = base + __popc(emask & ((1u << lane) - 1u));
+        const uint32_t d = (qz ? (uint32_t)__ldcg(qz + (qid >> 1)) : z) - rem;
         if (pos < arena_cap) arena[pos] = BcRawHit{qid, kf, kf + s - 1u, d};
         atomicAdd(&qcnt[qid], 1u);
     }
@@ -186,19 +190,19 @@ __device__ __forceinline__ uint32_t q_base(const uint8_t *rec, uint32_t boff, ui
     return c;
 }
 
-// First position at which a state with d = dc, seed differences sdc can afford ANY difference: before it
-// the D / Ds bounds (or a spent seed budget) leave exact matching as the only move.  dc == z: the read's end.
-// A value that is too SMALL only sends the state to a branch step early, which applies every rule itself.
-//   mismatch / insertion at t need D[t+1] <= z-dc-1, i.e. t >= thrD[z-dc-1] - 1 (deletions one later);
+// First position at which a state with `rem` differences left, seed differences sdc can afford ANY difference:
+// before it the D / Ds bounds (or a spent seed budget) leave exact matching as the only move.  rem == 0: the
+// read's end.  A value that is too SMALL only sends the state to a branch step early, which applies every rule itself.
+//   mismatch / insertion at t need D[t+1] <= rem-1, i.e. t >= thrD[rem-1] - 1 (deletions one later);
 //   inside the seed also sdc < seed_z and Ds[t+1] <= seed_z-sdc-1.
 // With E == 0 a deletion may precede W[0] outside the seed rule and follow W[m-1]; runs are then used for
 // spent budgets only (tests only; every config has E = 5).
 template <bool SMALL>
-__device__ __forceinline__ uint32_t run_end(const QThr &q, int dc, int sdc, int z, int seed_z, bool seed_on,
+__device__ __forceinline__ uint32_t run_end(const QThr &q, int rem, int sdc, int seed_z, bool seed_on,
                                             uint32_t seed_len, uint32_t m, bool e0, uint32_t soff) {
-    if (dc >= z) return m;
+    if (rem <= 0) return m;
     if (e0) return 0u;
-    uint32_t te = thr_d<SMALL>(q, z - dc - 1);
+    uint32_t te = thr_d<SMALL>(q, rem - 1);
     te = te ? te - 1u : 0u;
     if (seed_on) {
         uint32_t ts = seed_len;
@@ -223,8 +227,8 @@ template <bool S0, bool HAS_N, int LD>
 __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4 *lines, uint32_t primary,
                                             const uint32_t *Cs, uint2 *Cq, uint32_t CCAP, uint32_t &cnt,
                                             bool drain, uint2 *P, uint32_t bb, uint32_t &bcnt, uint32_t BCAP,
-                                            unsigned long long *ctr, uint32_t &n_nodes, uint32_t &n_xsect,
-                                            uint32_t &n_steps) {
+                                            unsigned long long *ctr, uint32_t z, const uint8_t *qz, uint32_t &n_nodes,
+                                            uint32_t &n_xsect, uint32_t &n_steps) {
     const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u, BM = BCAP - 1u;
     while ((cnt >= 32u || (drain && cnt > 0u)) && bcnt + 32u <= BCAP) {
         const uint32_t a = cnt < 32u ? cnt : 32u;
@@ -285,9 +289,46 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
             ent_store(P, (bb + bcnt + __popc(rmask & lt_mask)) & BM, qid, k, s, k2, (mlo & 0x07FFF800u) | t, mhi & 0x00FFFFFFu);
         bcnt += __popc(rmask);
         if (__any_sync(0xffffffffu, emit))
-            emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, S0 ? k2 : k, s, (mhi >> 8) & 255u);
+            emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, S0 ? k2 : k, s, (mhi >> 8) & 255u, z, qz);
         __syncwarp();
     }
+}
+
+// Root states of up to 32 queries (one per lane, `want`), each with `budget` differences to spend: dropped if its
+// D[0] / Ds[0] bounds already exceed the budgets, else pushed on the branch ring or -- when no
+// difference is affordable at W[0] -- on its strand's run stack.  The caller guarantees room for 32 entries.
+template <bool SMALL, bool HAS_N>
+__device__ __forceinline__ void push_roots(const BcSearchParams &p, bool want, uint32_t q, int budget, uint2 *P, uint32_t bb,
+                                           uint32_t &bcnt, uint32_t BM, uint2 *Cq, uint32_t CCAP, uint32_t &c0, uint32_t &c1,
+                                           bool e0) {
+    const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u;
+    const uint32_t full = p.ix.bwt[0].n + 1;
+    const int seed_len = p.o.seed_len, seed_z = p.o.seed_z;
+    bool ok = want;
+    uint32_t m = 0, te = 0, b0 = 0;
+    if (ok) {
+        m = p.reads.len[q >> 1];
+        ok = m >= 1 && m <= p.reads.max_len;
+    }
+    if (ok) {
+        const uint8_t *rec = p.ws.qrec + (size_t)q * p.ws.qstride;
+        const QThr th = load_thr<SMALL>(rec);
+        const bool seed_on = seed_len > 0 && seed_len < (int)m;
+        ok = thr_d<SMALL>(th, budget) == 0u && (!seed_on || thr_s<SMALL>(th, seed_z, p.ws.q_soff) == 0u);
+        te = run_end<SMALL>(th, budget, 0, seed_z, seed_on, (uint32_t)seed_len, m, e0, p.ws.q_soff);
+        b0 = q_base<HAS_N>(rec, p.ws.q_boff, p.ws.q_noff, 0u);
+    }
+    const bool odd = (q & 1u) != 0, run = ok && te > 0u;
+    const uint32_t maskb = __ballot_sync(0xffffffffu, ok && !run);
+    const uint32_t mask1 = __ballot_sync(0xffffffffu, run && odd), mask0 = __ballot_sync(0xffffffffu, run && !odd);
+    const uint32_t hi = ((uint32_t)budget << 8) | ((m - 1u) << 16);
+    if (ok) {
+        if (!run) ent_store(P, (bb + bcnt + __popc(maskb & lt_mask)) & BM, q, 0u, full, 0u, 0u, hi);
+        else ent_store(Cq, odd ? c1 + __popc(mask1 & lt_mask) : CCAP - 1u - c0 - __popc(mask0 & lt_mask), q,
+                       0u, full, 0u, b0 << 27, hi | ((te - 1u) << 24));
+    }
+    bcnt += __popc(maskb); c1 += __popc(mask1); c0 += __popc(mask0);
+    __syncwarp();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -314,6 +355,7 @@ template <bool SMALL, bool HAS_N, int LD>
 __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
+    __shared__ uint32_t cta_poller;                                          // this CTA has a warp that takes donated work
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
     uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
@@ -324,15 +366,28 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     const int z = p.o.z, E = p.o.indel_end_skip, max_go = p.o.max_gap_open, max_ge = p.o.max_gap_ext;
     const int seed_len = p.o.seed_len, seed_z = p.o.seed_z;
     const bool e0 = E == 0;
-    const uint32_t nq = p.ws.nq;
+    const uint32_t nq = p.ws.nq, n_reads = p.ws.nq >> 1;
     const uint32_t full = p.ix.bwt[0].n + 1;
+    const bool best = p.best != 0;                  // best-stratum mode: per-read budgets in qz[]
+    const uint8_t *qz = best ? p.ws.qz : nullptr;
+    uint32_t my_read = 0, my_bud = 0, my_st = 0, max_bud = 0;   // best mode: this lane's read, its budget, 0 free / 1 searching / 2 final round
     const uint32_t qstride = p.ws.qstride, soff = p.ws.q_soff, boff = p.ws.q_boff, noff = p.ws.q_noff;
     unsigned long long *ctr = (unsigned long long *)p.ws.ctr;
     const uint4 *lines0 = p.ix.bwt[1].lines, *lines1 = p.ix.bwt[0].lines;  // strand 0 searches the reverse index
     const uint32_t primary0 = p.ix.bwt[1].primary, primary1 = p.ix.bwt[0].primary;
 
     if (threadIdx.x < 8) Ctab[threadIdx.x] = p.ix.bwt[threadIdx.x < 4 ? 1 : 0].C[threadIdx.x & 3];
+    if (threadIdx.x == 0) cta_poller = 0u;
     __syncthreads();
+    // A4, state-level redistribution ACROSS warps (exhaustive mode): a busy warp that is about to spill the bottom of
+    // its ring gives that block of 32 pending states away instead, if some warp has run out of work; the first
+    // idle warp of every CTA stays behind as its CTA's "poller" and takes such blocks.  See steal_* below.
+#define QN (p.best ? 0u : p.ws.sq_n)                /* read from the parameter bank where needed: no register */
+#define sq_flag ((volatile uint32_t *)p.ws.sq_flag)  /* per slot: 0 free, 3 being written, 1 ready, 2 being read */
+    bool is_poller = false, counted_idle = false;
+    // warps that have STARTED: with more CTAs in the grid than fit on the machine the others start only when these
+    // leave, so "everybody idle" must mean everybody who runs (a late CTA finds no tickets and no blocks, and leaves)
+    if (lane == 0 && QN) atomicAdd(&ctr[BC_CTR_STARTED], 1ull);
     uint32_t bb = 1u << 24, bcnt = 0, c0 = 0, c1 = 0, gsp = 0, gsp_max = 0, pool_max = 0;   // ring bottom, counts (branch, run per strand), spilled blocks
     bool more = true, force_drain = false;
     // 32-bit statistics, flushed to the 64-bit global counters at every intake and at the end
@@ -340,12 +395,34 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 
     for (;;) {
         // ---- ring <-> global: keep the hot top of the branch stack on chip, >= 64 slots free ----------
-        while (bcnt >= 32u && bcnt + 64u > BCAP && gsp < GB) {               // spill the bottom 32 entries
+        while (bcnt >= 32u && bcnt + 64u > BCAP) {                             // move the bottom 32 entries out
             const uint2 *src = P + ((bb + lane) & BM) * 3u;
-            uint2 *dst = G + ((size_t)gsp * 32u + lane) * 3u;
-            dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
-            bb += 32u; bcnt -= 32u; ++gsp; ++n_spill;
-            gsp_max = gsp > gsp_max ? gsp : gsp_max;
+            uint32_t slot = 0xFFFFFFFFu;
+            if (QN) {                                                          // somebody idle?  give the block away
+                if (lane == 0 && *(volatile unsigned long long *)&ctr[BC_CTR_GIDLE] > 0ull)
+                    for (uint32_t a = 0; a < 4u && slot == 0xFFFFFFFFu; ++a) {
+                        const uint32_t s_ = ((blockIdx.x * 8u + warp) * 7u + a * 61u + n_spill + gsp + bb) % QN;
+                        if (atomicCAS(const_cast<uint32_t *>(&sq_flag[s_]), 0u, 3u) == 0u) slot = s_;
+                    }
+                slot = __shfl_sync(0xffffffffu, slot, 0);
+            }
+            if (slot != 0xFFFFFFFFu) {
+                uint2 *dst = p.ws.sq_buf + ((size_t)slot * 32u + lane) * 3u;
+                dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) {
+                    atomicExch(const_cast<uint32_t *>(&sq_flag[slot]), 1u);
+                    atomicAdd(&ctr[BC_CTR_QREADY], 1ull);
+                }
+            } else {
+                if (gsp >= GB) break;
+                uint2 *dst = G + ((size_t)gsp * 32u + lane) * 3u;
+                dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+                ++gsp; ++n_spill;
+                gsp_max = gsp > gsp_max ? gsp : gsp_max;
+            }
+            bb += 32u; bcnt -= 32u;
             __syncwarp();
         }
         if (bcnt < 32u && gsp > 0u) {                                          // bring the last block back
@@ -356,59 +433,144 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             bcnt += 32u;
             __syncwarp();
         }
-        // ---- intake: new root states while the branch stack is shallow ------------------------
-        if (more && bcnt < 32u && gsp == 0u && c0 + c1 + 32u <= CCAP) {
+        // ---- intake: new root states ---------------------------------------------------------------
+        if (!best) {
+            // exhaustive mode: new queries whenever the branch stack is shallow
+            if (more && bcnt < 32u && gsp == 0u && c0 + c1 + 32u <= CCAP) {
+                flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+                n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
+                uint32_t need = 32u - bcnt;
+                unsigned long long tk = 0;
+                if (lane == 0) {
+                    // towards the end of the batch take fewer queries at a time, so that the last heavy
+                    // trees are spread over the warps instead of queueing behind one another
+                    const unsigned long long seen = *(volatile unsigned long long *)&ctr[BC_CTR_TICKET];
+                    const unsigned long long left = seen < nq ? nq - seen : 0ull;
+                    const unsigned long long fair = left / (4ull * gridDim.x * (blockDim.x >> 5)) + 1ull;
+                    if (fair < need) need = (uint32_t)fair;
+                    tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
+                }
+                need = __shfl_sync(0xffffffffu, need, 0);
+                tk = __shfl_sync(0xffffffffu, tk, 0);
+                if (tk + need >= nq) more = false;
+                const unsigned long long q = tk + lane;
+                push_roots<SMALL, HAS_N>(p, lane < need && q < nq, (uint32_t)q, z, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0);
+            }
+        } else if (bcnt == 0u && c0 + c1 == 0u && gsp == 0u) {
+            // best-stratum mode: one read per lane, searched with ITS OWN budget, round by round.  All of
+            // the warp's trees are finished here, so each lane can judge its read by the raw hits counted so far:
+            //   no hit yet  -> same read again with budget + 1 (up to z);
+            //   first hits  -> they all have d = budget = d_min; one more round at min(d_min + plus, z) if that is
+            //                  larger (its hits are exactly the wanted set; the earlier ones are in it: duplicates
+            //                  with equal d, which the dedup of A6 removes), else done.
+            // Free lanes draw new reads.  Nothing with d > d_min + plus is ever explored.
             flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
-            uint32_t need = 32u - bcnt;
-            unsigned long long tk = 0;
-            if (lane == 0) {
-                // towards the end of the batch take fewer queries at a time, so that the last heavy
-                // trees are spread over the warps instead of queueing behind one another
-                const unsigned long long seen = *(volatile unsigned long long *)&ctr[BC_CTR_TICKET];
-                const unsigned long long left = seen < nq ? nq - seen : 0ull;
-                const unsigned long long fair = left / (4ull * gridDim.x * (blockDim.x >> 5)) + 1ull;
-                if (fair < need) need = (uint32_t)fair;
-                tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
+            if (my_st) {
+                const uint32_t h = *(volatile uint32_t *)&p.ws.qcnt[2u * my_read] + *(volatile uint32_t *)&p.ws.qcnt[2u * my_read + 1u];
+                if (my_st == 2u) my_st = 0u;
+                else if (h > 0u) {
+                    const uint32_t zf = my_bud + (uint32_t)p.plus < (uint32_t)z ? my_bud + (uint32_t)p.plus : (uint32_t)z;
+                    if (zf > my_bud) { my_bud = zf; my_st = 2u; } else my_st = 0u;
+                } else if (my_bud < (uint32_t)z) ++my_bud;
+                else my_st = 0u;
             }
-            need = __shfl_sync(0xffffffffu, need, 0);
-            tk = __shfl_sync(0xffffffffu, tk, 0);
-            if (tk + need >= nq) more = false;
-            unsigned long long q = tk + lane;
-            bool ok = lane < need && q < nq;
-            uint32_t m = 0, te = 0, b0 = 0;
-            if (ok) {
-                m = p.reads.len[q >> 1];
-                ok = m >= 1 && m <= p.reads.max_len;
+            const uint32_t freemask = __ballot_sync(0xffffffffu, my_st == 0u);
+            if (more && freemask) {
+                uint32_t need = __popc(freemask);
+                unsigned long long tk = 0;
+                if (lane == 0) {
+                    const unsigned long long seen = *(volatile unsigned long long *)&ctr[BC_CTR_TICKET];
+                    const unsigned long long left = seen < n_reads ? n_reads - seen : 0ull;
+                    const unsigned long long fair = left / (4ull * gridDim.x * (blockDim.x >> 5)) + 1ull;
+                    if (fair < need) need = (uint32_t)fair;
+                    tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);     // tickets are READS in this mode
+                }
+                need = __shfl_sync(0xffffffffu, need, 0);
+                tk = __shfl_sync(0xffffffffu, tk, 0);
+                if (tk + need >= n_reads) more = false;
+                const uint32_t rank = __popc(freemask & lt_mask);
+                if (my_st == 0u && rank < need && tk + rank < n_reads) { my_read = (uint32_t)(tk + rank); my_bud = 0u; my_st = 1u; }
             }
-            if (ok) {
-                const uint8_t *rec = p.ws.qrec + (size_t)q * qstride;
-                const QThr th = load_thr<SMALL>(rec);
-                const bool seed_on = seed_len > 0 && seed_len < (int)m;
-                // D[0] <= z and Ds[0] <= seed_z, else nothing can align
-                ok = thr_d<SMALL>(th, z) == 0u && (!seed_on || thr_s<SMALL>(th, seed_z, soff) == 0u);
-                te = run_end<SMALL>(th, 0, 0, z, seed_z, seed_on, (uint32_t)seed_len, m, e0, soff);
-                b0 = q_base<HAS_N>(rec, boff, noff, 0u);
-            }
-            const bool odd = (q & 1ull) != 0, run = ok && te > 0u;
-            const uint32_t maskb = __ballot_sync(0xffffffffu, ok && !run);
-            const uint32_t mask1 = __ballot_sync(0xffffffffu, run && odd), mask0 = __ballot_sync(0xffffffffu, run && !odd);
-            if (ok) {
-                if (!run) ent_store(P, (bb + bcnt + __popc(maskb & lt_mask)) & BM, (uint32_t)q, 0u, full, 0u, 0u, (m - 1) << 16);
-                else ent_store(Cq, odd ? c1 + __popc(mask1 & lt_mask) : CCAP - 1u - c0 - __popc(mask0 & lt_mask), (uint32_t)q,
-                               0u, full, 0u, b0 << 27, ((m - 1) << 16) | ((te - 1u) << 24));
-            }
-            bcnt += __popc(maskb); c1 += __popc(mask1); c0 += __popc(mask0);
+            if (!__any_sync(0xffffffffu, my_st != 0u)) { if (!more) break; continue; }
+            if (my_st) { __stcg(const_cast<uint8_t *>(qz) + my_read, (uint8_t)my_bud); max_bud = my_bud > max_bud ? my_bud : max_bud; }
             __syncwarp();
+            push_roots<SMALL, HAS_N>(p, my_st != 0u, 2u * my_read + 1u, (int)my_bud, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0);
+            push_roots<SMALL, HAS_N>(p, my_st != 0u, 2u * my_read, (int)my_bud, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0);
         }
-        if (bcnt == 0 && c0 + c1 == 0) { if (!more) break; continue; }
+        if (bcnt == 0 && c0 + c1 == 0) {
+            if (more || best) continue;               // (best mode: the round logic above decides when the warp is done)
+            if (!QN) break;
+            // ---- out of work.  Count this warp idle; the first idle warp of the CTA becomes its poller, the others leave.
+            flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+            n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
+            if (!is_poller) {
+                uint32_t won = 0;
+                if (lane == 0) won = atomicCAS(&cta_poller, 0u, 1u) == 0u ? 1u : 0u;
+                is_poller = __shfl_sync(0xffffffffu, won, 0) != 0u;
+            }
+            if (lane == 0) { __threadfence(); atomicAdd(&ctr[BC_CTR_GIDLE], 1ull); }
+            counted_idle = true;
+            if (!is_poller) break;
+            // ---- poller: take donated blocks until every warp is idle and nothing is left in the exchange.
+            // A thief un-counts itself BEFORE it tries to claim, so "all idle" (read first) followed by "nothing ready"
+            // (read second) means every published block was claimed by a warp that will come back here.
+            bool got = false;
+            uint32_t spins = 0;
+            for (;;) {
+                unsigned long long idle = 0, ready = 0, err = 0, started = 0;
+                if (lane == 0) {
+                    started = *(volatile unsigned long long *)&ctr[BC_CTR_STARTED];
+                    idle = *(volatile unsigned long long *)&ctr[BC_CTR_GIDLE];
+                    __threadfence();
+                    ready = *(volatile unsigned long long *)&ctr[BC_CTR_QREADY];
+                    err = *(volatile unsigned long long *)&ctr[BC_CTR_ERROR];
+                }
+                idle = __shfl_sync(0xffffffffu, idle, 0); ready = __shfl_sync(0xffffffffu, ready, 0);
+                err = __shfl_sync(0xffffffffu, err, 0); started = __shfl_sync(0xffffffffu, started, 0);
+                if (err) break;
+                if (++spins > (1u << 28)) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // ~10 min: a bug, not a wait
+                if (ready > 0ull) {
+                    if (lane == 0) atomicAdd(&ctr[BC_CTR_GIDLE], ~0ull);                  // -1: not idle while claiming
+                    uint32_t slot = 0xFFFFFFFFu;
+                    for (uint32_t base = 0; base < QN && slot == 0xFFFFFFFFu; base += 32u) {
+                        const uint32_t s_ = ((blockIdx.x * 8u + warp) * 13u + base + lane) % QN;
+                        uint32_t mk = __ballot_sync(0xffffffffu, sq_flag[s_] == 1u);
+                        while (mk && slot == 0xFFFFFFFFu) {
+                            const int l = __ffs(mk) - 1;
+                            mk &= mk - 1u;
+                            const uint32_t cand = __shfl_sync(0xffffffffu, s_, l);
+                            uint32_t ok = 0;
+                            if (lane == 0) ok = atomicCAS(const_cast<uint32_t *>(&sq_flag[cand]), 1u, 2u) == 1u ? 1u : 0u;
+                            if (__shfl_sync(0xffffffffu, ok, 0)) slot = cand;
+                        }
+                    }
+                    if (slot != 0xFFFFFFFFu) {
+                        if (lane == 0) atomicAdd(&ctr[BC_CTR_QREADY], ~0ull);
+                        const uint2 *src = p.ws.sq_buf + ((size_t)slot * 32u + lane) * 3u;
+                        uint2 *dst = P + ((bb + lane) & BM) * 3u;
+                        dst[0] = __ldcg(src); dst[1] = __ldcg(src + 1); dst[2] = __ldcg(src + 2);
+                        bcnt = 32u;
+                        __syncwarp();
+                        if (lane == 0) { __threadfence(); atomicExch(const_cast<uint32_t *>(&sq_flag[slot]), 0u); atomicAdd(&ctr[BC_CTR_STEALS], 1ull); }
+                        counted_idle = false;
+                        got = true;
+                        break;
+                    }
+                    if (lane == 0) atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);
+                } else if (idle >= started) break;
+                __nanosleep(2000);
+            }
+            if (!got) break;
+            continue;
+        }
         pool_max = bcnt + c0 + c1 > pool_max ? bcnt + c0 + c1 : pool_max;
 
         if (c1 >= 32u || c0 >= 32u || ((bcnt == 0 || force_drain) && c0 + c1 > 0u)) {
             if (bcnt + 32u > BCAP) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 4ull); break; }   // spill area exhausted
             const bool drain = bcnt == 0 || force_drain;
-            chain_steps<false, HAS_N, LD>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
-            chain_steps<true, HAS_N, LD>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, n_cnodes, n_xsect, n_csteps);
+            chain_steps<false, HAS_N, LD>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, (uint32_t)z, qz, n_cnodes, n_xsect, n_csteps);
+            chain_steps<true, HAS_N, LD>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, (uint32_t)z, qz, n_cnodes, n_xsect, n_csteps);
             force_drain = false;
             continue;
         }
@@ -425,7 +587,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         __syncwarp();
 
         const int t = mlo & 511, st = (mlo >> 9) & 3, go = (mlo >> 11) & 255, ge = (mlo >> 19) & 255;
-        const int sd = mhi & 255, d = (mhi >> 8) & 255, m = (int)((mhi >> 16) & 255) + 1;
+        const int sd = mhi & 255, rem = (mhi >> 8) & 255, m = (int)((mhi >> 16) & 255) + 1;
         const uint32_t strand = qid & 1u;
         const bool seed_on = seed_len > 0 && seed_len < m;
         const bool has_base = act && t < m;
@@ -461,12 +623,12 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         const int in_seed_del = (seed_on && t > 0 && t < seed_len) ? 1 : 0;
         const uint32_t m_bits = mhi & 0x00FF0000u;
         // class-level validity and packed child state (same for every child of a class).  A child that costs a
-        // difference has d+1 = nd1 and needs D <= z - nd1 at ITS position: t+1 for mismatch / insertion, t for a
+        // difference has rem-1 = nrem left and needs D <= nrem at ITS position: t+1 for mismatch / insertion, t for a
         // deletion; inside the seed the same with Ds and the seed budget (zero thresholds outside / seed off).
-        const int nd1 = d + 1, sdb = sd + in_seed_base, sdd = sd + in_seed_del;
+        const int nrem = rem - 1, sdb = sd + in_seed_base, sdd = sd + in_seed_del;
         const uint32_t tn = (uint32_t)t + 1u;
-        const bool bud = act && nd1 <= z;
-        const uint32_t thD = bud ? thr_d<SMALL>(th, z - nd1) : 0u;
+        const bool bud = act && rem >= 1;
+        const uint32_t thD = bud ? thr_d<SMALL>(th, nrem) : 0u;
         const bool v_base = bud && has_base && sdb <= seed_z && tn >= thD && tn >= thr_s<SMALL>(th, sdb <= seed_z ? seed_z - sdb : 0, soff);
         const int d_go = go + (st != 2), d_ge = ge + (st == 2), i_go = go + (st != 1), i_ge = ge + (st == 1);
         const bool v_mm = v_base;
@@ -474,18 +636,19 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         const bool v_del = bud && del_ok && d_go <= max_go && d_ge <= max_ge && sdd <= seed_z && (uint32_t)t >= thD &&
                            (uint32_t)t >= thr_s<SMALL>(th, sdd <= seed_z ? seed_z - sdd : 0, soff);
         // where the children go: the end of the run a child starts with (te > its position: run stack)
-        const uint32_t te_b = run_end<SMALL>(th, nd1, sdb, z, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
+        const uint32_t te_b = run_end<SMALL>(th, nrem, sdb, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
         const uint32_t te_d = in_seed_del == in_seed_base ? te_b
-                              : run_end<SMALL>(th, nd1, sdd, z, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
+                              : run_end<SMALL>(th, nrem, sdd, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
         const bool run_b = te_b > tn, run_d = te_d > (uint32_t)t;
+        const uint32_t nrem8 = (uint32_t)(nrem & 255) << 8;
         const uint32_t ma_lo = tn | ((uint32_t)go << 11) | ((uint32_t)ge << 19);
-        const uint32_t ma_hi = (uint32_t)sd | ((uint32_t)d << 8) | m_bits;
-        const uint32_t mm_hi = (uint32_t)sdb | ((uint32_t)nd1 << 8) | m_bits | (run_b ? (te_b - 1u) << 24 : 0u);
+        const uint32_t ma_hi = (uint32_t)sd | ((uint32_t)rem << 8) | m_bits;
+        const uint32_t mm_hi = (uint32_t)sdb | nrem8 | m_bits | (run_b ? (te_b - 1u) << 24 : 0u);
         const uint32_t de_lo = (uint32_t)t | (2u << 9) | ((uint32_t)d_go << 11) | ((uint32_t)d_ge << 19);
-        const uint32_t de_hi = (uint32_t)sdd | ((uint32_t)nd1 << 8) | m_bits | (run_d ? (te_d - 1u) << 24 : 0u);
+        const uint32_t de_hi = (uint32_t)sdd | nrem8 | m_bits | (run_d ? (te_d - 1u) << 24 : 0u);
         const uint32_t in_lo = tn | (1u << 9) | ((uint32_t)i_go << 11) | ((uint32_t)i_ge << 19);
         const uint32_t cb0 = run_d ? qb << 27 : 0u, cb1 = run_b ? qb1 << 27 : 0u;   // first base of a run child
-        const bool last1 = nd1 == z;                     // children that cost a difference exhaust the budget
+        const bool last1 = nrem == 0;                    // children that cost a difference exhaust the budget
         const bool term_base = (int)tn == m;             // children that consume W[t] finish the read
         const bool term_del = t == m;
 
@@ -577,16 +740,20 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                 uint32_t ck2 = sel4(nk2[0], nk2[1], nk2[2], nk2[3], b);
                 if (slot == 9) { ck = k; cs = s; ck2 = k2; }
                 emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, em, qid, strand ? ck : ck2, cs,
-                          (uint32_t)(slot == 0 ? d : nd1));
+                          (uint32_t)(slot == 0 ? rem : nrem), (uint32_t)z, qz);
             }
         }
         __syncwarp();
     }
     flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+    if (QN && !counted_idle && lane == 0) atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);    // error exits: pollers must not wait for this warp
     if (lane == 0) {
         atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
         atomicMax(&ctr[BC_CTR_SPILLMAX], (unsigned long long)gsp_max);
     }
+    if (best) atomicMax(&ctr[BC_CTR_PASSES], (unsigned long long)max_bud + 1ull);
+#undef QN
+#undef sq_flag
 }
 
 template <bool SMALL, bool HAS_N, int LD>

@@ -36,12 +36,18 @@ enum {                      // indices into the uint64 counter block
     BC_CTR_CANCEL = 13,     // branch states popped and put back because their children did not fit
     BC_CTR_SPILL = 14,      // 32-entry blocks moved from the branch rings to global memory
     BC_CTR_SPILLMAX = 15,   // deepest per-warp spill stack seen (blocks)
-    BC_CTR_COUNT = 16
+    BC_CTR_PASSES = 16,     // best-stratum mode: largest per-read budget searched + 1
+    BC_CTR_GIDLE = 17,      // warps that are out of work (state exchange between warps)
+    BC_CTR_QREADY = 18,     // donated blocks waiting in the exchange
+    BC_CTR_STEALS = 19,     // blocks of 32 states that changed warps
+    BC_CTR_STARTED = 20,    // warps that have started (the exchange waits for these, not for the whole grid)
+    BC_CTR_COUNT = 24
 };
 
 struct BcRawHit { uint32_t qid, k, l, d; };
 
 struct BcWorkspace {        // device pointers into the caller's workspace
+    uint8_t *qz;            // [n_reads] best-stratum mode: the budget each read is being searched with
     uint8_t *qrec;          // [nq][qstride] prepared query records (layout above)
     uint32_t qstride, q_soff, q_boff, q_noff;
     uint32_t *qcnt;         // [nq] raw hits per query
@@ -57,6 +63,9 @@ struct BcWorkspace {        // device pointers into the caller's workspace
     uint64_t arena_cap;
     uint2 *spill;           // [warps in the grid][spill_blocks][32 entries][3] overflow of the branch rings
     uint32_t spill_blocks;  // blocks of 32 entries per warp
+    uint32_t *sq_flag;      // [sq_n] state exchange between warps: slot states (zeroed per call)
+    uint2 *sq_buf;          // [sq_n][32 entries][3]
+    uint32_t sq_n;          // slots (multiple of 32; 0 = exchange off)
     uint32_t nq;
 };
 
@@ -67,6 +76,7 @@ struct BcSearchParams {
     BcWorkspace ws;
     uint32_t bcap;          // branch ring entries per warp (power of two)
     uint32_t ccap;          // run stack entries per warp (both strands)
+    uint32_t best, plus;    // best-stratum mode (bc_align_batch_best): per read only the hits with d <= min(d_min + plus, z)
     uint32_t ld_policy;     // 0 = default cache policies for the index loads, 1 = no L1 allocation + 64 B L2 prefetch size
 };
 
@@ -79,4 +89,5 @@ cudaError_t bc_exclusive_scan(const uint32_t *in, uint64_t n, uint64_t *blk, uin
                               cudaStream_t st);
 // smem bytes one pool entry takes; used by the host to size pools
 #define BC_POOL_ENTRY_BYTES 24u
+#define BC_STEAL_SLOTS 256u           // blocks in flight between warps (768 B each)
 #define BC_SPILL_BLOCKS 128u          // per warp: 128 x 32 entries x 24 B = 96 KB of workspace

@@ -256,6 +256,31 @@ def test_result_independent_of_kernel_geometry():
     assert st["nodes"] > 0 and st["lookups"] == 2 * st["nodes"]
 
 
+def test_states_move_between_warps_and_results_do_not():
+    """A4: a small batch of heavy trees (config 5a's options: 36 bp, z=4, no seed) leaves most warps without
+    queries; busy warps give the bottom of their ring away, pollers take it.  The CSR must be byte-identical
+    with the exchange on (blocks did move), off, and to the oracle."""
+    cfg, p = pair_for("5a", 1_000_000)
+    reads = sd.make_reads(cfg.scaled(n_reads=400), p.T, 0, 400)
+    opts = cfg.opts.astuple()
+    rl = list(reads.codes)
+    outs, steals = [], []
+    try:
+        for geo, pol in [((0, 0), 0), ((0, 0), 256), ((2, 8), 0), ((5, 2), 0)]:
+            bc.bc_set_geometry(p.ix, *geo)
+            bc.bc_set_tuning(p.ix, 0, 0, pol)
+            off, hits = gpu_align(p.ix, rl, opts)
+            outs.append((off.tobytes(), hits.tobytes()))
+            steals.append(bc.bc_last_stats(p.ix)["passes_or_steals"])
+    finally:
+        bc.bc_set_geometry(p.ix, 0, 0)
+        bc.bc_set_tuning(p.ix, 0, 0, 0)
+    assert all(o == outs[0] for o in outs)
+    assert steals[0] > 0 and steals[1] == 0 and steals[2] > 0
+    off_o, hits_o = p.oracle.align(reads.codes, opts)
+    assert outs[0] == (off_o.tobytes(), hits_o.tobytes())
+
+
 def test_status_codes_for_small_buffers_and_deep_budgets():
     cfg, p = pair_for("1", sd.CONFIGS["1"].n)
     reads = [p.T[10:46].copy()]
@@ -331,7 +356,7 @@ def test_moderately_deep_budget():
 
 
 def test_autotune_keeps_parity_as_a_hard_constraint():
-    from paper_1505_07855_b200.autotune import autotune_geometry
+    from paper_1505_07855_b200.autotune import autotune_geometry, autotune, GENES
     cfg, p = pair_for("2", 2_000_000)
     reads = sd.make_reads(cfg.scaled(n_reads=4000), p.T, 0, 4000)
     opts = cfg.opts.astuple()
@@ -343,3 +368,9 @@ def test_autotune_keeps_parity_as_a_hard_constraint():
     off_o, hits_o = p.oracle.align(reads.codes, opts)
     bc.bc_set_geometry(p.ix, 0, 0)
     assert np.array_equal(off_g, off_o) and hits_g.tobytes() == hits_o.tobytes()
+    # the evolutionary search over the run-time genes (build-time genes need the compiler; see profiles/r02_autotune_*)
+    runtime = {k: v for k, v in GENES.items() if k != "min_ctas"}
+    runtime["min_ctas"] = (GENES["min_ctas"][0],)
+    best, table = autotune(p.host, bc.HostReads(b2, nm, off, ln), opts, budget=6, repeats=1, genes=runtime)
+    ok = [r for r in table if r["status"] == "ok"]
+    assert len(table) == 6 and ok and all(r["identical"] for r in ok) and best["search_ms"] <= table[0]["search_ms"]
