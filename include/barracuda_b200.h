@@ -185,9 +185,11 @@ int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
  * states (default 128; bc_align_batch returns BC_E_NOMEM when a warp's area runs full -- raise it, ask
  * bc_align_workspace_bytes again and repeat the call); pool_kb = shared memory per SM given to the
  * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond); ld_policy = cache
- * policy of the index loads, 1 = default, 2 = no L1 allocation + 64-byte L2 prefetch size (default: 1 for
- * an index up to 64 MB, 2 beyond); ld_policy + 256 switches the exchange of pending states between warps
- * off (A/B measurements).  spill_blocks affects the workspace size: set it before bc_align_workspace_bytes. */
+ * policy of the index loads: 1 = default policies, 2 = no L1 allocation + 64-byte L2 prefetch size (the library
+ * default), 3 = as 2 plus an L2 eviction priority by interval width (wide intervals = the top of the search
+ * trees evict-last, the rest evict-first; intervals of >= n >> s rows are wide, s = (ld_policy >> 9) & 31,
+ * 0 = 16); ld_policy + 256 switches the exchange of pending states between warps off (A/B measurements).
+ * spill_blocks affects the workspace size: set it before bc_align_workspace_bytes. */
 int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb, uint32_t ld_policy);
 
 /* Host-side index construction for synthetic genomes (untimed helper): suffix sort

@@ -28,7 +28,7 @@ GENES = {                                   # value 0 = "library default" for th
     "ctas": (0, 2, 3, 4, 5, 6),             # CTAs per SM launched
     "warps": (0, 4, 6, 8),                  # warps per CTA
     "pool_kb": (0, 128, 144, 160, 176, 192, 208),   # shared memory per SM given to the state pools
-    "ld_policy": (0, 1, 2),                 # cache policy of the index loads
+    "ld_policy": (0, 1, 2, 3),              # cache policy of the index loads (bc_set_tuning)
 }
 DEFAULT = {k: v[0] for k, v in GENES.items()}
 

@@ -61,10 +61,10 @@ int choose_geometry(const bc_index *ix, Geometry &g) {
     g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
     g.spill_blocks = ix->spill_blocks ? ix->spill_blocks : BC_SPILL_BLOCKS;
     for (;; --g.ctas) {
-        // pool bytes per SM; what is left of the 228 KB stays L1 (index sectors, query records).  Round 1, measured:
-        // config 2 (16 MB index, L2-resident) 144/160/176/192/208/220 KB -> 101.5/98.0/96.7/95.5/98.1/99.1 ms;
-        // configs 3 and 4 (index >= L2) 2-3 % faster at 160 than at 192 (L2 misses make L1 count)
-        const size_t total_kb = ix->pool_kb ? ix->pool_kb : (ix->bytes > ((size_t)64 << 20) ? 160 : 192);
+        // pool bytes per SM; what is left of the 228 KB stays L1 (query records).  The autotuner's tables
+        // (profiles/r02_autotune_config2.json, _config4.json): 16 MB index 160/176/192 KB -> 92.6/90.3/89.3 ms;
+        // 1.5 GB index 160/176 KB -> 254.4/252.2 ms (L2 misses make L1 count for more there)
+        const size_t total_kb = ix->pool_kb ? ix->pool_kb : (ix->bytes > ((size_t)64 << 20) ? 176 : 192);
         size_t budget = total_kb * 1024 / g.ctas;
         if (budget > 200 * 1024) budget = 200 * 1024;
         uint32_t per_warp = (uint32_t)(budget / ((size_t)g.warps * BC_POOL_ENTRY_BYTES));
@@ -164,7 +164,9 @@ int bc_align_impl(const bc_index *ix_c, const bc_reads *reads, const bc_opts *o,
     p.ccap = g.ccap;
     p.best = best_plus >= 0 ? 1u : 0u;
     p.plus = best_plus >= 0 ? (uint32_t)best_plus : 0u;
-    p.ld_policy = ix->ld_policy ? ix->ld_policy - 1u : (ix->bytes > ((size_t)64 << 20) ? 1u : 0u);
+    p.ld_policy = ix->ld_policy ? ix->ld_policy - 1u : 1u;     // autotuner: no L1 allocation wins at every index size
+    p.wide_s = (uint32_t)(ix->n >> (ix->wide_shift ? ix->wide_shift : 16u));
+    if (p.wide_s < 64u) p.wide_s = 64u;
     ws.spill = (uint2 *)(base + L.off_spill);
     ws.spill_blocks = L.spill_blocks;
 

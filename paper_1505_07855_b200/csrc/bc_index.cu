@@ -140,7 +140,7 @@ extern "C" int bc_index_upload(const bc_index_host *h, void *d_mem, size_t d_byt
     ix->dev.sa_interval = h->sa_interval;
     ix->n = n;
     ix->bytes = L.total;
-    ix->ctas_per_sm = 0; ix->warps_per_cta = 0; ix->spill_blocks = 0; ix->pool_kb = 0; ix->ld_policy = 0; ix->no_exchange = 0;
+    ix->ctas_per_sm = 0; ix->warps_per_cta = 0; ix->spill_blocks = 0; ix->pool_kb = 0; ix->ld_policy = 0; ix->no_exchange = 0; ix->wide_shift = 0;
     ix->h_ctr = nullptr;
     for (int i = 0; i < 16; ++i) ix->stats[i] = 0;
     int dev = 0, sms = 0;
@@ -192,12 +192,13 @@ extern "C" int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warp
 }
 
 extern "C" int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb, uint32_t ld_policy) {
-    if (!ix || spill_blocks > 65536 || (pool_kb != 0 && (pool_kb < 16 || pool_kb > 220)) || (ld_policy & 255u) > 2 || ld_policy > 511u)
+    if (!ix || spill_blocks > 65536 || (pool_kb != 0 && (pool_kb < 16 || pool_kb > 220)) || (ld_policy & 255u) > 3 || ld_policy > 0x3FFFu)
         return BC_E_INVAL;
     ix->spill_blocks = spill_blocks;
     ix->pool_kb = pool_kb;
     ix->ld_policy = ld_policy & 255u;
     ix->no_exchange = (ld_policy >> 8) & 1u;
+    ix->wide_shift = (ld_policy >> 9) & 31u;
     return BC_OK;
 }
 

@@ -45,7 +45,8 @@ struct bc_index {            // the opaque handle of the ABI
     uint32_t ctas_per_sm, warps_per_cta;   // 0 = chosen by the library (bc_set_geometry)
     uint32_t spill_blocks;   // per-warp spill area of the branch rings, blocks of 32 states (bc_set_tuning)
     uint32_t pool_kb;        // shared memory per SM given to the state pools, 0 = by index size (bc_set_tuning)
-    uint32_t ld_policy;      // cache policy of the index loads: 0 = by index size, 1 = default, 2 = no L1 / 64 B L2
+    uint32_t ld_policy;      // cache policy of the index loads: 0 = library default, 1..3 = LD 0..2 of bc_load_block
+    uint32_t wide_shift;     // LD 2: intervals of >= n >> wide_shift rows count as the top of the trees (0 = 16)
     uint32_t no_exchange;    // 1 = warps keep their states to themselves (bc_set_tuning ld_policy bit 8: A/B measurements)
     uint64_t stats[16];
     int sm_count;
@@ -62,17 +63,30 @@ __device__ __forceinline__ uint32_t bc_rank_pos(const BcBwtDev &b, uint32_t x) {
 
 struct BcBlockRegs { uint32_t c0, c1, c2, c3; uint64_t lo, hi; };
 
-// The one load that carries the whole search, with two cache policies (chosen per index size by the host,
-// bc_set_tuning; measured on the 1 Gbp index: L1 hit rate of index sectors 9 %, +5 % reads/s with policy 1):
-//   LD = 0  read-only path, default policies          (index resident in L2: L1 helps the top of the trees)
-//   LD = 1  read-only path, no L1 allocation, 64-byte L2 prefetch size (index far beyond L2)
+// The one load that carries the whole search, with three cache policies (bc_set_tuning; the defaults are the
+// autotuner's result, profiles/r02_autotune_*):
+//   LD = 0  read-only path, default policies
+//   LD = 1  read-only path, no L1 allocation, 64-byte L2 prefetch size (index lines hit L1 9 % of the time; not
+//           allocating them leaves L1 to the query records: -9 % time on config 2, -3..5 % on config 4)
+//   LD = 2  as 1, plus an L2 eviction priority by interval width: `wide` (the top of the search trees, which every
+//           query walks) evict-last, the rest evict-first -- random deep lines turn the 126 MB L2 over every ~25 us
+//           and would otherwise push the shared top levels out
 // one 256-bit read-only load of the block that holds position p of the '$'-less string
 template <int LD = 0>
-__device__ __forceinline__ BcBlockRegs bc_load_block(const uint4 *lines, uint32_t p) {
+__device__ __forceinline__ BcBlockRegs bc_load_block(const uint4 *lines, uint32_t p, bool wide = false) {
     const uint4 *q = lines + (size_t)(p >> 6) * 2;
     BcBlockRegs r;
     uint32_t l0, l1, h0, h1;
-    if (LD == 1)
+    if (LD == 2) {
+        if (wide)
+            asm("ld.global.nc.L1::no_allocate.L2::evict_last.L2::64B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
+                : "l"(q));
+        else
+            asm("ld.global.nc.L1::no_allocate.L2::evict_first.L2::64B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
+                : "l"(q));
+    } else if (LD == 1)
         asm("ld.global.nc.L1::no_allocate.L2::64B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
             : "=r"(r.c0), "=r"(r.c1), "=r"(r.c2), "=r"(r.c3), "=r"(l0), "=r"(l1), "=r"(h0), "=r"(h1)
             : "l"(q));
@@ -99,8 +113,8 @@ __device__ __forceinline__ void bc_block_rank4(const BcBlockRegs &r, uint32_t p,
 
 // all four O(., .) before position p of the '$'-less string
 template <int LD = 0>
-__device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_t out[4]) {
-    bc_block_rank4(bc_load_block<LD>(lines, p), p, out);
+__device__ __forceinline__ void bc_rank4(const uint4 *lines, uint32_t p, uint32_t out[4], bool wide = false) {
+    bc_block_rank4(bc_load_block<LD>(lines, p, wide), p, out);
 }
 
 // one symbol's count from a loaded block: #{j < p : B'[j] = c}  (c > 3 gives a don't-care value)

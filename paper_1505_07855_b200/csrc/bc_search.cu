@@ -106,8 +106,11 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 //   mhi = seed_d (0-7) | rem (8-15) | m-1 (16-23);  rem = the query's budget - d, the differences still affordable
 //         (the kernel never needs d itself except when a hit is emitted: d = budget - rem)
 //   run entries also carry the base they match next (mlo bits 27-29) and the end of their run - 1 (mhi 24-31)
+//   mlo bit 30 (BC_FREE_BIT): this state may change warps (always in the exhaustive mode; best-stratum mode: only
+//   states of a read's LAST round, whose outcome no verdict waits for)
 // Per warp: a RING of BRANCH states (some difference is affordable at their position), whose cold bottom
 // spills to global memory in blocks of 32, and two stacks of RUN states (see the kernel's comment).
+#define BC_FREE_BIT 0x40000000u
 #ifndef BC_SEARCH_MAX_THREADS
 #define BC_SEARCH_MAX_THREADS 256
 #endif
@@ -249,7 +252,7 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             const bool two = (plo >> 6) != (phi >> 6);
-            const BcBlockRegs rlo = bc_load_block<LD>(lines, plo);
+            const BcBlockRegs rlo = bc_load_block<LD>(lines, plo, s >= p.wide_s);
             n_xsect += two ? 1u : 0u;
             // strand 0 also needs one OTHER symbol's count for the forward start k2 (see below):
             // x = A when c is A or C, x = T when c is G or T
@@ -257,7 +260,7 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
             uint32_t olo = bc_block_rank1(rlo, plo, c), ohi, xlo = 0, xhi = 0;
             if (S0) xlo = bc_block_rank1(rlo, plo, x);
             if (two) {                                    // most narrow intervals sit in one sector
-                const BcBlockRegs rhi = bc_load_block<LD>(lines, phi);
+                const BcBlockRegs rhi = bc_load_block<LD>(lines, phi, s >= p.wide_s);
                 ohi = bc_block_rank1(rhi, phi, c);
                 if (S0) xhi = bc_block_rank1(rhi, phi, x);
             } else {
@@ -281,12 +284,12 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
         const uint32_t smask = __ballot_sync(0xffffffffu, alive);
         if (alive) {
             const uint32_t r = __popc(smask & lt_mask);
-            ent_store(Cq, S0 ? CCAP - 1u - cnt - r : cnt + r, qid, k, s, k2, (mlo & 0x07FFFE00u) | t | (nb << 27), mhi);
+            ent_store(Cq, S0 ? CCAP - 1u - cnt - r : cnt + r, qid, k, s, k2, (mlo & 0x47FFFE00u) | t | (nb << 27), mhi);
         }
         cnt += __popc(smask);
         const uint32_t rmask = __ballot_sync(0xffffffffu, toring);
         if (toring)      // a run consists of matches: gap state M, budgets unchanged
-            ent_store(P, (bb + bcnt + __popc(rmask & lt_mask)) & BM, qid, k, s, k2, (mlo & 0x07FFF800u) | t, mhi & 0x00FFFFFFu);
+            ent_store(P, (bb + bcnt + __popc(rmask & lt_mask)) & BM, qid, k, s, k2, (mlo & 0x47FFF800u) | t, mhi & 0x00FFFFFFu);
         bcnt += __popc(rmask);
         if (__any_sync(0xffffffffu, emit))
             emit_hits(p.ws.arena, p.ws.arena_cap, p.ws.qcnt, ctr, emit, qid, S0 ? k2 : k, s, (mhi >> 8) & 255u, z, qz);
@@ -300,7 +303,7 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
 template <bool SMALL, bool HAS_N>
 __device__ __forceinline__ void push_roots(const BcSearchParams &p, bool want, uint32_t q, int budget, uint2 *P, uint32_t bb,
                                            uint32_t &bcnt, uint32_t BM, uint2 *Cq, uint32_t CCAP, uint32_t &c0, uint32_t &c1,
-                                           bool e0) {
+                                           bool e0, bool free_state) {
     const uint32_t lane = threadIdx.x & 31u, lt_mask = (1u << lane) - 1u;
     const uint32_t full = p.ix.bwt[0].n + 1;
     const int seed_len = p.o.seed_len, seed_z = p.o.seed_z;
@@ -323,9 +326,10 @@ __device__ __forceinline__ void push_roots(const BcSearchParams &p, bool want, u
     const uint32_t mask1 = __ballot_sync(0xffffffffu, run && odd), mask0 = __ballot_sync(0xffffffffu, run && !odd);
     const uint32_t hi = ((uint32_t)budget << 8) | ((m - 1u) << 16);
     if (ok) {
-        if (!run) ent_store(P, (bb + bcnt + __popc(maskb & lt_mask)) & BM, q, 0u, full, 0u, 0u, hi);
+        const uint32_t fb = free_state ? BC_FREE_BIT : 0u;
+        if (!run) ent_store(P, (bb + bcnt + __popc(maskb & lt_mask)) & BM, q, 0u, full, 0u, fb, hi);
         else ent_store(Cq, odd ? c1 + __popc(mask1 & lt_mask) : CCAP - 1u - c0 - __popc(mask0 & lt_mask), q,
-                       0u, full, 0u, b0 << 27, hi | ((te - 1u) << 24));
+                       0u, full, 0u, (b0 << 27) | fb, hi | ((te - 1u) << 24));
     }
     bcnt += __popc(maskb); c1 += __popc(mask1); c0 += __popc(mask0);
     __syncwarp();
@@ -356,6 +360,9 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
     __shared__ uint32_t cta_poller;                                          // this CTA has a warp that takes donated work
+    // rarely touched per-lane / per-warp variables live in shared memory, not in registers of the hot loop:
+    __shared__ uint2 best_lane[BC_SEARCH_MAX_THREADS];                       // best mode: {read, budget | state << 8} of this lane's read
+    __shared__ uint32_t warp_flags[BC_SEARCH_MAX_THREADS / 32];              // bit 0 poller, 1 counted idle, 2 best mode done
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
     uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
@@ -370,7 +377,6 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     const uint32_t full = p.ix.bwt[0].n + 1;
     const bool best = p.best != 0;                  // best-stratum mode: per-read budgets in qz[]
     const uint8_t *qz = best ? p.ws.qz : nullptr;
-    uint32_t my_read = 0, my_bud = 0, my_st = 0, max_bud = 0;   // best mode: this lane's read, its budget, 0 free / 1 searching / 2 final round
     const uint32_t qstride = p.ws.qstride, soff = p.ws.q_soff, boff = p.ws.q_boff, noff = p.ws.q_noff;
     unsigned long long *ctr = (unsigned long long *)p.ws.ctr;
     const uint4 *lines0 = p.ix.bwt[1].lines, *lines1 = p.ix.bwt[0].lines;  // strand 0 searches the reverse index
@@ -382,13 +388,18 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
     // A4, state-level redistribution ACROSS warps (exhaustive mode): a busy warp that is about to spill the bottom of
     // its ring gives that block of 32 pending states away instead, if some warp has run out of work; the first
     // idle warp of every CTA stays behind as its CTA's "poller" and takes such blocks.  See steal_* below.
-#define QN (p.best ? 0u : p.ws.sq_n)                /* read from the parameter bank where needed: no register */
+#define QN (p.ws.sq_n)                                /* read from the parameter bank where needed: no register */
 #define sq_flag ((volatile uint32_t *)p.ws.sq_flag)  /* per slot: 0 free, 3 being written, 1 ready, 2 being read */
-    bool is_poller = false, counted_idle = false;
+    best_lane[threadIdx.x] = make_uint2(0u, 0u);     // state 0 free / 1 searching for the first hit / 2 final round
+    if (lane == 0) warp_flags[warp] = 0u;
+    __syncwarp();
+#define WF_POLLER 1u
+#define WF_COUNTED 2u
+#define WF_BESTDONE 4u
     // warps that have STARTED: with more CTAs in the grid than fit on the machine the others start only when these
     // leave, so "everybody idle" must mean everybody who runs (a late CTA finds no tickets and no blocks, and leaves)
     if (lane == 0 && QN) atomicAdd(&ctr[BC_CTR_STARTED], 1ull);
-    uint32_t bb = 1u << 24, bcnt = 0, c0 = 0, c1 = 0, gsp = 0, gsp_max = 0, pool_max = 0;   // ring bottom, counts (branch, run per strand), spilled blocks
+    uint32_t bb = 1u << 24, bcnt = 0, c0 = 0, c1 = 0, gsp = 0, pool_max = 0;   // ring bottom, counts (branch, run per strand), spilled blocks
     bool more = true, force_drain = false;
     // 32-bit statistics, flushed to the 64-bit global counters at every intake and at the end
     uint32_t n_cnodes = 0, n_xsect = 0, n_bsteps = 0, n_bnodes = 0, n_csteps = 0, n_cancel = 0, n_spill = 0;
@@ -399,7 +410,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             const uint2 *src = P + ((bb + lane) & BM) * 3u;
             uint32_t slot = 0xFFFFFFFFu;
             if (QN) {                                                          // somebody idle?  give the block away
-                if (lane == 0 && *(volatile unsigned long long *)&ctr[BC_CTR_GIDLE] > 0ull)
+                const bool all_free = __all_sync(0xffffffffu, (src[2].x & BC_FREE_BIT) != 0u);
+                if (lane == 0 && all_free && *(volatile unsigned long long *)&ctr[BC_CTR_GIDLE] > 0ull)
                     for (uint32_t a = 0; a < 4u && slot == 0xFFFFFFFFu; ++a) {
                         const uint32_t s_ = ((blockIdx.x * 8u + warp) * 7u + a * 61u + n_spill + gsp + bb) % QN;
                         if (atomicCAS(const_cast<uint32_t *>(&sq_flag[s_]), 0u, 3u) == 0u) slot = s_;
@@ -420,7 +432,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                 uint2 *dst = G + ((size_t)gsp * 32u + lane) * 3u;
                 dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
                 ++gsp; ++n_spill;
-                gsp_max = gsp > gsp_max ? gsp : gsp_max;
+                if (lane == 0 && (gsp & 7u) == 0u) atomicMax(&ctr[BC_CTR_SPILLMAX], (unsigned long long)gsp);   // (to a multiple of 8)
             }
             bb += 32u; bcnt -= 32u;
             __syncwarp();
@@ -454,7 +466,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                 tk = __shfl_sync(0xffffffffu, tk, 0);
                 if (tk + need >= nq) more = false;
                 const unsigned long long q = tk + lane;
-                push_roots<SMALL, HAS_N>(p, lane < need && q < nq, (uint32_t)q, z, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0);
+                push_roots<SMALL, HAS_N>(p, lane < need && q < nq, (uint32_t)q, z, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0, true);
             }
         } else if (bcnt == 0u && c0 + c1 == 0u && gsp == 0u) {
             // best-stratum mode: one read per lane, searched with ITS OWN budget, round by round.  All of
@@ -466,6 +478,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             // Free lanes draw new reads.  Nothing with d > d_min + plus is ever explored.
             flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
+            uint32_t my_read = best_lane[threadIdx.x].x, my_bud = best_lane[threadIdx.x].y & 255u, my_st = best_lane[threadIdx.x].y >> 8;
             if (my_st) {
                 const uint32_t h = *(volatile uint32_t *)&p.ws.qcnt[2u * my_read] + *(volatile uint32_t *)&p.ws.qcnt[2u * my_read + 1u];
                 if (my_st == 2u) my_st = 0u;
@@ -492,26 +505,32 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                 const uint32_t rank = __popc(freemask & lt_mask);
                 if (my_st == 0u && rank < need && tk + rank < n_reads) { my_read = (uint32_t)(tk + rank); my_bud = 0u; my_st = 1u; }
             }
-            if (!__any_sync(0xffffffffu, my_st != 0u)) { if (!more) break; continue; }
-            if (my_st) { __stcg(const_cast<uint8_t *>(qz) + my_read, (uint8_t)my_bud); max_bud = my_bud > max_bud ? my_bud : max_bud; }
+            best_lane[threadIdx.x] = make_uint2(my_read, my_bud | (my_st << 8));
+            if (!__any_sync(0xffffffffu, my_st != 0u)) { if (more) continue; if (lane == 0) warp_flags[warp] |= WF_BESTDONE; __syncwarp(); }
+            else {
+            if (my_st) __stcg(const_cast<uint8_t *>(qz) + my_read, (uint8_t)my_bud);
+            { const uint32_t mb = __reduce_max_sync(0xffffffffu, my_st ? my_bud + 1u : 0u); if (lane == 0) atomicMax(&ctr[BC_CTR_PASSES], (unsigned long long)mb); }
             __syncwarp();
-            push_roots<SMALL, HAS_N>(p, my_st != 0u, 2u * my_read + 1u, (int)my_bud, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0);
-            push_roots<SMALL, HAS_N>(p, my_st != 0u, 2u * my_read, (int)my_bud, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0);
+            // a round after which the read is done whatever it finds (its final round, or budget z) may share its states
+            const bool last_round = my_st == 2u || my_bud >= (uint32_t)z;
+            push_roots<SMALL, HAS_N>(p, my_st != 0u, 2u * my_read + 1u, (int)my_bud, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0, last_round);
+            push_roots<SMALL, HAS_N>(p, my_st != 0u, 2u * my_read, (int)my_bud, P, bb, bcnt, BM, Cq, CCAP, c0, c1, e0, last_round);
+            }
         }
         if (bcnt == 0 && c0 + c1 == 0) {
-            if (more || best) continue;               // (best mode: the round logic above decides when the warp is done)
+            if (more || (best && !(warp_flags[warp] & WF_BESTDONE))) continue;   // (best mode: the round logic above decides when the warp is done)
             if (!QN) break;
             // ---- out of work.  Count this warp idle; the first idle warp of the CTA becomes its poller, the others leave.
             flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
-            if (!is_poller) {
-                uint32_t won = 0;
-                if (lane == 0) won = atomicCAS(&cta_poller, 0u, 1u) == 0u ? 1u : 0u;
-                is_poller = __shfl_sync(0xffffffffu, won, 0) != 0u;
+            if (lane == 0) {
+                if (!(warp_flags[warp] & WF_POLLER) && atomicCAS(&cta_poller, 0u, 1u) == 0u) warp_flags[warp] |= WF_POLLER;
+                __threadfence();
+                atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);
+                warp_flags[warp] |= WF_COUNTED;
             }
-            if (lane == 0) { __threadfence(); atomicAdd(&ctr[BC_CTR_GIDLE], 1ull); }
-            counted_idle = true;
-            if (!is_poller) break;
+            __syncwarp();
+            if (!(warp_flags[warp] & WF_POLLER)) break;
             // ---- poller: take donated blocks until every warp is idle and nothing is left in the exchange.
             // A thief un-counts itself BEFORE it tries to claim, so "all idle" (read first) followed by "nothing ready"
             // (read second) means every published block was claimed by a warp that will come back here.
@@ -553,7 +572,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                         bcnt = 32u;
                         __syncwarp();
                         if (lane == 0) { __threadfence(); atomicExch(const_cast<uint32_t *>(&sq_flag[slot]), 0u); atomicAdd(&ctr[BC_CTR_STEALS], 1ull); }
-                        counted_idle = false;
+                        if (lane == 0) warp_flags[warp] &= ~WF_COUNTED;
                         got = true;
                         break;
                     }
@@ -608,8 +627,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             uint32_t olo[4], ohi[4];
-            bc_rank4<LD>(lines, plo, olo);                   // two unconditional loads: predicating the second one on
-            bc_rank4<LD>(lines, phi, ohi);                   // "other sector" was measured 3 % slower here (not in the run step)
+            bc_rank4<LD>(lines, plo, olo, s >= p.wide_s);                   // two unconditional loads: predicating the second one on
+            bc_rank4<LD>(lines, phi, ohi, s >= p.wide_s);                   // "other sector" was measured 3 % slower here (not in the run step)
             straddle = (plo >> 6) != (phi >> 6);
             const uint4 Cv = *reinterpret_cast<const uint4 *>(Ctab + strand * 4u);
             const uint32_t Cc[4] = {Cv.x, Cv.y, Cv.z, Cv.w};
@@ -641,12 +660,13 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                               : run_end<SMALL>(th, nrem, sdd, seed_z, seed_on, (uint32_t)seed_len, (uint32_t)m, e0, soff);
         const bool run_b = te_b > tn, run_d = te_d > (uint32_t)t;
         const uint32_t nrem8 = (uint32_t)(nrem & 255) << 8;
-        const uint32_t ma_lo = tn | ((uint32_t)go << 11) | ((uint32_t)ge << 19);
+        const uint32_t fb = mlo & BC_FREE_BIT;
+        const uint32_t ma_lo = tn | ((uint32_t)go << 11) | ((uint32_t)ge << 19) | fb;
         const uint32_t ma_hi = (uint32_t)sd | ((uint32_t)rem << 8) | m_bits;
         const uint32_t mm_hi = (uint32_t)sdb | nrem8 | m_bits | (run_b ? (te_b - 1u) << 24 : 0u);
-        const uint32_t de_lo = (uint32_t)t | (2u << 9) | ((uint32_t)d_go << 11) | ((uint32_t)d_ge << 19);
+        const uint32_t de_lo = (uint32_t)t | (2u << 9) | ((uint32_t)d_go << 11) | ((uint32_t)d_ge << 19) | fb;
         const uint32_t de_hi = (uint32_t)sdd | nrem8 | m_bits | (run_d ? (te_d - 1u) << 24 : 0u);
-        const uint32_t in_lo = tn | (1u << 9) | ((uint32_t)i_go << 11) | ((uint32_t)i_ge << 19);
+        const uint32_t in_lo = tn | (1u << 9) | ((uint32_t)i_go << 11) | ((uint32_t)i_ge << 19) | fb;
         const uint32_t cb0 = run_d ? qb << 27 : 0u, cb1 = run_b ? qb1 << 27 : 0u;   // first base of a run child
         const bool last1 = nrem == 0;                    // children that cost a difference exhaust the budget
         const bool term_base = (int)tn == m;             // children that consume W[t] finish the read
@@ -746,14 +766,15 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         __syncwarp();
     }
     flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
-    if (QN && !counted_idle && lane == 0) atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);    // error exits: pollers must not wait for this warp
+    if (QN && lane == 0 && !(warp_flags[warp] & WF_COUNTED)) atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);    // error exits: pollers must not wait for this warp
     if (lane == 0) {
         atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
-        atomicMax(&ctr[BC_CTR_SPILLMAX], (unsigned long long)gsp_max);
     }
-    if (best) atomicMax(&ctr[BC_CTR_PASSES], (unsigned long long)max_bud + 1ull);
 #undef QN
 #undef sq_flag
+#undef WF_POLLER
+#undef WF_COUNTED
+#undef WF_BESTDONE
 }
 
 template <bool SMALL, bool HAS_N, int LD>
@@ -766,6 +787,7 @@ cudaError_t launch_search(const BcSearchParams &p, int grid, int threads, size_t
 
 template <bool SMALL, bool HAS_N>
 cudaError_t launch_search_ld(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
+    if (p.ld_policy == 2) return launch_search<SMALL, HAS_N, 2>(p, grid, threads, smem, st);
     return p.ld_policy ? launch_search<SMALL, HAS_N, 1>(p, grid, threads, smem, st) : launch_search<SMALL, HAS_N, 0>(p, grid, threads, smem, st);
 }
 
