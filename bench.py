@@ -451,7 +451,7 @@ def run_ours(args):
 
     # ---- measured random-access rates (the metric's own denominator), outside the timed region ----
     if not args.no_probe:
-        idx_bytes = 2 * (cfg.n // 64 + 1) * 32
+        idx_bytes = int(out["config"]["index_bytes"])
         rs_res = bc.bc_measure_random_sectors(min(idx_bytes, 8 << 30), 512, dev)
         rs_hbm = bc.bc_measure_random_sectors(8 << 30, 256, dev)
         sect_s = stats["lines"] / k_s if k_s else 0.0

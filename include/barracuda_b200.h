@@ -167,10 +167,10 @@ int bc_pair_batch(const bc_index *ix, const uint64_t *d_hit_offsets, const bc_hi
 int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint32_t *d_pos, void *cuda_stream);
 
 /* Device-side counters of the last bc_align_batch on this index (HOST out array of 16 uint64):
- * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] distinct 32-byte index blocks (sectors) fetched,
+ * [0] search nodes expanded, [1] Occ lookups (rank queries), [2] 32-byte index sectors the rank queries read (1 per unit for blocks, 2 for lines),
  * [3] raw hits, [4] D-kernel lookups, [5] pool high-water mark, [6] search-kernel ns (CUDA events
  * on the caller's stream around the persistent search kernel), [7] geometry used:
- * ctas_per_sm << 32 | warps_per_cta << 16 | pool entries per warp, [8] warp-level branch steps,
+ * ctas_per_sm << 32 | warps_per_cta << 16 | index layout << 15 | pool entries per warp, [8] warp-level branch steps,
  * [9] nodes expanded in branch steps, [10] warp-level chain iterations, [11] nodes expanded in
  * chain iterations, [12] branch states popped and put back because their children did not fit,
  * [13] 32-entry blocks of branch states spilled from the on-chip rings to the workspace,
@@ -186,11 +186,15 @@ int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
  * bc_align_workspace_bytes again and repeat the call); pool_kb = shared memory per SM given to the
  * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond); ld_policy = cache
  * policy of the index loads: 1 = default policies, 2 = no L1 allocation + 64-byte L2 prefetch size (the library
- * default), 3 = as 2 plus an L2 eviction priority by interval width (wide intervals = the top of the search
- * trees evict-last, the rest evict-first; intervals of >= n >> s rows are wide, s = (ld_policy >> 9) & 31,
- * 0 = 16); ld_policy + 256 switches the exchange of pending states between warps off (A/B measurements).
+ * default); ld_policy + 256 switches the exchange of pending states between warps off (A/B measurements).
  * spill_blocks affects the workspace size: set it before bc_align_workspace_bytes. */
 int bc_set_tuning(bc_index *ix, uint32_t spill_blocks, uint32_t pool_kb, uint32_t ld_policy);
+
+/* Device layout of indexes uploaded from now on (process-wide; 0 = by size, the default: 32-byte blocks of 64
+ * symbols while the index fits 64 MB, 128-byte lines of 384 symbols beyond -- on B200 a missing 32-byte sector
+ * costs a whole 128-byte line of DRAM traffic, so an index that lives in HBM makes the line its unit; 1 = blocks,
+ * 2 = lines).  Read by bc_index_device_bytes and bc_index_upload.  Results do not depend on it. */
+int bc_set_index_layout(int choice);
 
 /* Host-side index construction for synthetic genomes (untimed helper): suffix sort
  * of T$ and reverse(T)$ -> transport arrays.  text: HOST, n codes 0..3.  The arrays are allocated

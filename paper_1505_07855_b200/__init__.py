@@ -101,6 +101,7 @@ def lib():
         L.bc_last_stats.argtypes = [vp, C.POINTER(u64 * 16)]
         L.bc_set_geometry.argtypes = [vp, u32, u32]
         L.bc_set_tuning.argtypes = [vp, u32, u32, u32]
+        L.bc_set_index_layout.argtypes = [i32]
         L.bc_index_build_host.argtypes = [vp, u64, u32, u32, i32, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_index_host_free.argtypes = [C.POINTER(bc_index_host)]
         L.bc_index_build_gpu_bytes.argtypes = [u64, u32, u32, C.POINTER(C.c_size_t)]
@@ -109,7 +110,7 @@ def lib():
         L.bc_strerror.argtypes = [i32]
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
-                  "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_set_tuning", "bc_index_build_host",
+                  "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_set_tuning", "bc_set_index_layout", "bc_index_build_host",
                   "bc_index_host_free", "bc_measure_random_sectors", "bc_align_best_workspace_bytes",
                   "bc_align_batch_best", "bc_pair_workspace_bytes", "bc_pair_batch", "bc_index_build_gpu_bytes", "bc_index_build_gpu"):
             getattr(L, f).restype = i32
@@ -287,6 +288,11 @@ def bc_index_upload(h: HostIndex, device="cuda:0", stream=None) -> DeviceIndex:
 
 def bc_set_geometry(ix: DeviceIndex, ctas_per_sm: int = 0, warps_per_cta: int = 0):
     _check(lib().bc_set_geometry(ix.handle, ctas_per_sm, warps_per_cta), "bc_set_geometry")
+
+
+def bc_set_index_layout(choice: int = 0):
+    """Device layout of indexes uploaded from now on: 0 by size, 1 = 32-byte blocks, 2 = 128-byte lines."""
+    _check(lib().bc_set_index_layout(choice), "bc_set_index_layout")
 
 
 def bc_set_tuning(ix: DeviceIndex, spill_blocks: int = 0, pool_kb: int = 0, ld_policy: int = 0):

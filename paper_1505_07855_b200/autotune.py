@@ -28,7 +28,8 @@ GENES = {                                   # value 0 = "library default" for th
     "ctas": (0, 2, 3, 4, 5, 6),             # CTAs per SM launched
     "warps": (0, 4, 6, 8),                  # warps per CTA
     "pool_kb": (0, 128, 144, 160, 176, 192, 208),   # shared memory per SM given to the state pools
-    "ld_policy": (0, 1, 2, 3),              # cache policy of the index loads (bc_set_tuning)
+    "ld_policy": (0, 1, 2),                 # cache policy of the index loads (bc_set_tuning)
+    "layout": (0, 1, 2),                    # device index layout (bc_set_index_layout; needs a re-upload)
 }
 DEFAULT = {k: v[0] for k, v in GENES.items()}
 
@@ -46,18 +47,22 @@ class Evaluator:
         self.hreads, self.opts, self.device, self.repeats, self.best_plus = hreads, opts, device, repeats, best_plus
         self._lib_for, self._ix = None, None
 
-    def _index(self, min_ctas: int):
-        if self._lib_for != min_ctas:
+    def _index(self, min_ctas: int, layout: int):
+        if self._lib_for != (min_ctas, layout):
             if self._ix is not None:
                 self._ix.free()
             so = None if min_ctas == DEFAULT["min_ctas"] else _build.build_variant({"BC_SEARCH_MIN_CTAS": min_ctas})
             bc.use_library(so)
-            self._ix = bc.bc_index_upload(bc.HostIndex.from_arrays(self.arrays), self.device)
-            self._lib_for = min_ctas
+            bc.bc_set_index_layout(layout)
+            try:
+                self._ix = bc.bc_index_upload(bc.HostIndex.from_arrays(self.arrays), self.device)
+            finally:
+                bc.bc_set_index_layout(0)
+            self._lib_for = (min_ctas, layout)
         return self._ix
 
     def __call__(self, g: dict):
-        ix = self._index(g["min_ctas"])
+        ix = self._index(g["min_ctas"], g.get("layout", 0))
         bc.bc_set_geometry(ix, g["ctas"], g["warps"])
         bc.bc_set_tuning(ix, 0, g["pool_kb"], g["ld_policy"])
         d = self.hreads.to_device(self.device)

@@ -165,8 +165,6 @@ int bc_align_impl(const bc_index *ix_c, const bc_reads *reads, const bc_opts *o,
     p.best = best_plus >= 0 ? 1u : 0u;
     p.plus = best_plus >= 0 ? (uint32_t)best_plus : 0u;
     p.ld_policy = ix->ld_policy ? ix->ld_policy - 1u : 1u;     // autotuner: no L1 allocation wins at every index size
-    p.wide_s = (uint32_t)(ix->n >> (ix->wide_shift ? ix->wide_shift : 16u));
-    if (p.wide_s < 64u) p.wide_s = 64u;
     ws.spill = (uint2 *)(base + L.off_spill);
     ws.spill_blocks = L.spill_blocks;
 
@@ -193,7 +191,7 @@ int bc_align_impl(const bc_index *ix_c, const bc_reads *reads, const bc_opts *o,
     ix->stats[4] = ctr[BC_CTR_DLOOKUPS];
     ix->stats[5] = ctr[BC_CTR_POOLMAX];
     ix->stats[6] = (uint64_t)((double)ms * 1e6);
-    ix->stats[7] = (uint64_t)ctas << 32 | (uint64_t)warps << 16 | (g.bcap + g.ccap);
+    ix->stats[7] = (uint64_t)ctas << 32 | (uint64_t)warps << 16 | (uint64_t)ix->dev.bwt[0].layout << 15 | (g.bcap + g.ccap);
     ix->stats[8] = ctr[BC_CTR_BSTEPS];
     ix->stats[9] = ctr[BC_CTR_BNODES];
     ix->stats[10] = ctr[BC_CTR_CSTEPS];

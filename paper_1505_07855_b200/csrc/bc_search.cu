@@ -22,6 +22,7 @@ __device__ __forceinline__ uint32_t read_base(const bc_reads &rd, uint64_t pos) 
 // greedy piece count of SURVEY C7 over W[lo..hi), grown from W[hi-1] leftwards on the opposite-direction
 // index Y.  Whenever the count steps from c to c+1 at position a, D[a+1] = c is the last position with
 // D <= c: thr[c] = a+1 (thresholds beyond `rmax` are not needed; thr[] was zeroed: D[lo] <= r => 0).
+template <int LAY>
 __device__ __forceinline__ void piece_thresholds(const bc_reads &rd, uint64_t off, uint32_t strand, const BcBwtDev &Y,
                                                  int lo, int hi, int rmax, uint8_t *thr, uint64_t &lookups) {
     const uint32_t full = Y.n + 1;
@@ -31,7 +32,7 @@ __device__ __forceinline__ void piece_thresholds(const bc_reads &rd, uint64_t of
         if (c < 4 && strand) c = 3 - c;
         bool brk = c > 3;
         if (!brk) {
-            const uint32_t olo = bc_rank1(Y.lines, bc_rank_pos(Y, k), c), ohi = bc_rank1(Y.lines, bc_rank_pos(Y, k + s), c);
+            const uint32_t olo = bc_rank1<LAY>(Y.lines, bc_rank_pos(Y, k), c), ohi = bc_rank1<LAY>(Y.lines, bc_rank_pos(Y, k + s), c);
             lookups += 2;
             if (ohi == olo) brk = true; else { k = Y.C[c] + olo + 1; s = ohi - olo; }
         }
@@ -46,6 +47,7 @@ __device__ __forceinline__ void piece_thresholds(const bc_reads &rd, uint64_t of
 // A1 + A2: one thread per query (read, strand): writes the query record of bc_ws.cuh -- bases
 // (complemented for strand 1), N bits, and the D / Ds bounds as thresholds.
 // ---------------------------------------------------------------------------------------------
+template <int LAY>
 __global__ void bc_prepare_kernel(BcSearchParams p) {
     uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= p.ws.nq) return;
@@ -79,8 +81,8 @@ __global__ void bc_prepare_kernel(BcSearchParams p) {
     const BcBwtDev &Y = p.ix.bwt[strand ? 1 : 0];       // opposite direction of the search index
     const bool seed_on = p.o.seed_len > 0 && (uint32_t)p.o.seed_len < m;
     uint64_t lookups = 0;
-    if (seed_on) piece_thresholds(p.reads, off, strand, Y, 0, p.o.seed_len, p.o.seed_z, rec + p.ws.q_soff, lookups);
-    piece_thresholds(p.reads, off, strand, Y, 0, (int)m, p.o.z, rec, lookups);
+    if (seed_on) piece_thresholds<LAY>(p.reads, off, strand, Y, 0, p.o.seed_len, p.o.seed_z, rec + p.ws.q_soff, lookups);
+    piece_thresholds<LAY>(p.reads, off, strand, Y, 0, (int)m, p.o.z, rec, lookups);
     atomicAdd((unsigned long long *)&p.ws.ctr[BC_CTR_DLOOKUPS], (unsigned long long)lookups);
 }
 
@@ -88,7 +90,8 @@ __global__ void bc_prepare_kernel(BcSearchParams p) {
 
 cudaError_t bc_launch_prepare(const BcSearchParams &p, cudaStream_t st) {
     if (p.ws.nq == 0) return cudaSuccess;
-    bc_prepare_kernel<<<(p.ws.nq + 127) / 128, 128, 0, st>>>(p);
+    if (p.ix.bwt[0].layout == 0) bc_prepare_kernel<0><<<(p.ws.nq + 127) / 128, 128, 0, st>>>(p);
+    else bc_prepare_kernel<1><<<(p.ws.nq + 127) / 128, 128, 0, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -147,14 +150,14 @@ __device__ __noinline__ void emit_hits(BcRawHit *arena, unsigned long long arena
 // per-warp statistics: n_xsect is per lane (second sectors of a rank pair), the rest warp-uniform
 __device__ __noinline__ void flush_stats(unsigned long long *ctr, uint32_t lane, uint32_t n_cnodes, uint32_t n_xsect,
                                          uint32_t n_bsteps, uint32_t n_bnodes, uint32_t n_csteps, uint32_t n_cancel,
-                                         uint32_t n_spill) {
+                                         uint32_t n_spill, uint32_t sect) {
     uint32_t x = n_xsect;
     for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
     if (lane == 0) {
         const unsigned long long nodes = (unsigned long long)n_cnodes + n_bnodes;
         atomicAdd(&ctr[BC_CTR_NODES], nodes);
         atomicAdd(&ctr[BC_CTR_LOOKUPS], 2ull * nodes);
-        atomicAdd(&ctr[BC_CTR_LINES], nodes + x);          // one sector per node + the pairs that straddle two
+        atomicAdd(&ctr[BC_CTR_LINES], (nodes + x) * sect);   // rank units read (one per node + the pairs that straddle two) x sectors per unit
         atomicAdd(&ctr[BC_CTR_BSTEPS], (unsigned long long)n_bsteps);
         atomicAdd(&ctr[BC_CTR_BNODES], (unsigned long long)n_bnodes);
         atomicAdd(&ctr[BC_CTR_CSTEPS], (unsigned long long)n_csteps);
@@ -226,7 +229,7 @@ __device__ __forceinline__ uint32_t run_end(const QThr &q, int rem, int sdc, int
 // Stack layout inside the run area Cq[0..CCAP): strand 1 grows up from 0, strand 0 down from CCAP-1.
 // The caller guarantees 32 free ring slots per iteration (the loop re-checks).
 // ---------------------------------------------------------------------------------------------
-template <bool S0, bool HAS_N, int LD>
+template <bool S0, bool HAS_N, int LD, int LAY>
 __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4 *lines, uint32_t primary,
                                             const uint32_t *Cs, uint2 *Cq, uint32_t CCAP, uint32_t &cnt,
                                             bool drain, uint2 *P, uint32_t bb, uint32_t &bcnt, uint32_t BCAP,
@@ -251,21 +254,21 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
         if (act) {
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
-            const bool two = (plo >> 6) != (phi >> 6);
-            const BcBlockRegs rlo = bc_load_block<LD>(lines, plo, s >= p.wide_s);
+            const bool two = bc_unit_id<LAY>(plo) != bc_unit_id<LAY>(phi);
+            const BcUnit<LAY> rlo = bc_load_unit<LAY, LD>(lines, plo);
             n_xsect += two ? 1u : 0u;
             // strand 0 also needs one OTHER symbol's count for the forward start k2 (see below):
             // x = A when c is A or C, x = T when c is G or T
             const uint32_t x = c < 2u ? 0u : 3u;
-            uint32_t olo = bc_block_rank1(rlo, plo, c), ohi, xlo = 0, xhi = 0;
-            if (S0) xlo = bc_block_rank1(rlo, plo, x);
-            if (two) {                                    // most narrow intervals sit in one sector
-                const BcBlockRegs rhi = bc_load_block<LD>(lines, phi, s >= p.wide_s);
-                ohi = bc_block_rank1(rhi, phi, c);
-                if (S0) xhi = bc_block_rank1(rhi, phi, x);
+            uint32_t olo = bc_unit_rank1(rlo, plo, c), ohi, xlo = 0, xhi = 0;
+            if (S0) xlo = bc_unit_rank1(rlo, plo, x);
+            if (two) {                                    // most narrow intervals sit in one unit
+                const BcUnit<LAY> rhi = bc_load_unit<LAY, LD>(lines, phi);
+                ohi = bc_unit_rank1(rhi, phi, c);
+                if (S0) xhi = bc_unit_rank1(rhi, phi, x);
             } else {
-                ohi = bc_block_rank1(rlo, phi, c);
-                if (S0) xhi = bc_block_rank1(rlo, phi, x);
+                ohi = bc_unit_rank1(rlo, phi, c);
+                if (S0) xhi = bc_unit_rank1(rlo, phi, x);
             }
             if (c <= 3u && ohi != olo) {
                 if (S0) {
@@ -355,7 +358,7 @@ __device__ __forceinline__ void push_roots(const BcSearchParams &p, bool want, u
 // free and comes back when the ring runs low; if that area is ever full the warp raises error bit 2
 // (BC_E_NOMEM: the caller passes a larger spill area), never a silent truncation.
 // ---------------------------------------------------------------------------------------------
-template <bool SMALL, bool HAS_N, int LD>
+template <bool SMALL, bool HAS_N, int LD, int LAY>
 __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
@@ -449,7 +452,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         if (!best) {
             // exhaustive mode: new queries whenever the branch stack is shallow
             if (more && bcnt < 32u && gsp == 0u && c0 + c1 + 32u <= CCAP) {
-                flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+                flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill, bc_unit_sectors<LAY>());
                 n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
                 uint32_t need = 32u - bcnt;
                 unsigned long long tk = 0;
@@ -476,7 +479,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             //                  larger (its hits are exactly the wanted set; the earlier ones are in it: duplicates
             //                  with equal d, which the dedup of A6 removes), else done.
             // Free lanes draw new reads.  Nothing with d > d_min + plus is ever explored.
-            flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+            flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill, bc_unit_sectors<LAY>());
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             uint32_t my_read = best_lane[threadIdx.x].x, my_bud = best_lane[threadIdx.x].y & 255u, my_st = best_lane[threadIdx.x].y >> 8;
             if (my_st) {
@@ -521,7 +524,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             if (more || (best && !(warp_flags[warp] & WF_BESTDONE))) continue;   // (best mode: the round logic above decides when the warp is done)
             if (!QN) break;
             // ---- out of work.  Count this warp idle; the first idle warp of the CTA becomes its poller, the others leave.
-            flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+            flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill, bc_unit_sectors<LAY>());
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             if (lane == 0) {
                 if (!(warp_flags[warp] & WF_POLLER) && atomicCAS(&cta_poller, 0u, 1u) == 0u) warp_flags[warp] |= WF_POLLER;
@@ -588,8 +591,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         if (c1 >= 32u || c0 >= 32u || ((bcnt == 0 || force_drain) && c0 + c1 > 0u)) {
             if (bcnt + 32u > BCAP) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 4ull); break; }   // spill area exhausted
             const bool drain = bcnt == 0 || force_drain;
-            chain_steps<false, HAS_N, LD>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, (uint32_t)z, qz, n_cnodes, n_xsect, n_csteps);
-            chain_steps<true, HAS_N, LD>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, (uint32_t)z, qz, n_cnodes, n_xsect, n_csteps);
+            chain_steps<false, HAS_N, LD, LAY>(p, lines1, primary1, Ctab + 4, Cq, CCAP, c1, drain, P, bb, bcnt, BCAP, ctr, (uint32_t)z, qz, n_cnodes, n_xsect, n_csteps);
+            chain_steps<true, HAS_N, LD, LAY>(p, lines0, primary0, Ctab, Cq, CCAP, c0, drain, P, bb, bcnt, BCAP, ctr, (uint32_t)z, qz, n_cnodes, n_xsect, n_csteps);
             force_drain = false;
             continue;
         }
@@ -627,9 +630,14 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             const uint32_t x1 = k + s;
             const uint32_t plo = k - (k > primary ? 1u : 0u), phi = x1 - (x1 > primary ? 1u : 0u);
             uint32_t olo[4], ohi[4];
-            bc_rank4<LD>(lines, plo, olo, s >= p.wide_s);                   // two unconditional loads: predicating the second one on
-            bc_rank4<LD>(lines, phi, ohi, s >= p.wide_s);                   // "other sector" was measured 3 % slower here (not in the run step)
-            straddle = (plo >> 6) != (phi >> 6);
+            straddle = bc_unit_id<LAY>(plo) != bc_unit_id<LAY>(phi);
+            const BcUnit<LAY> ulo = bc_load_unit<LAY, LD>(lines, plo);
+            bc_unit_rank4(ulo, plo, olo);
+            if (LAY == 0) {                              // blocks: a second unconditional load (predicating it on "other
+                bc_unit_rank4(bc_load_unit<LAY, LD>(lines, phi), phi, ohi);   // block" was measured 3 % slower here)
+            } else if (straddle) {
+                bc_unit_rank4(bc_load_unit<LAY, LD>(lines, phi), phi, ohi);
+            } else bc_unit_rank4(ulo, phi, ohi);
             const uint4 Cv = *reinterpret_cast<const uint4 *>(Ctab + strand * 4u);
             const uint32_t Cc[4] = {Cv.x, Cv.y, Cv.z, Cv.w};
             uint32_t acc = k2 + s;                       // k2 + dollar + prefix, built below
@@ -765,7 +773,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         }
         __syncwarp();
     }
-    flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill);
+    flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill, bc_unit_sectors<LAY>());
     if (QN && lane == 0 && !(warp_flags[warp] & WF_COUNTED)) atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);    // error exits: pollers must not wait for this warp
     if (lane == 0) {
         atomicMax(&ctr[BC_CTR_POOLMAX], (unsigned long long)pool_max);
@@ -777,18 +785,19 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 #undef WF_BESTDONE
 }
 
-template <bool SMALL, bool HAS_N, int LD>
+template <bool SMALL, bool HAS_N, int LD, int LAY>
 cudaError_t launch_search(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N, LD, LAY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    bc_search_kernel<SMALL, HAS_N, LD><<<grid, threads, smem, st>>>(p);
+    bc_search_kernel<SMALL, HAS_N, LD, LAY><<<grid, threads, smem, st>>>(p);
     return cudaGetLastError();
 }
 
 template <bool SMALL, bool HAS_N>
 cudaError_t launch_search_ld(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
-    if (p.ld_policy == 2) return launch_search<SMALL, HAS_N, 2>(p, grid, threads, smem, st);
-    return p.ld_policy ? launch_search<SMALL, HAS_N, 1>(p, grid, threads, smem, st) : launch_search<SMALL, HAS_N, 0>(p, grid, threads, smem, st);
+    if (p.ix.bwt[0].layout == 0)
+        return p.ld_policy ? launch_search<SMALL, HAS_N, 1, 0>(p, grid, threads, smem, st) : launch_search<SMALL, HAS_N, 0, 0>(p, grid, threads, smem, st);
+    return p.ld_policy ? launch_search<SMALL, HAS_N, 1, 1>(p, grid, threads, smem, st) : launch_search<SMALL, HAS_N, 0, 1>(p, grid, threads, smem, st);
 }
 
 }  // namespace

@@ -77,8 +77,7 @@ struct BcSearchParams {
     uint32_t bcap;          // branch ring entries per warp (power of two)
     uint32_t ccap;          // run stack entries per warp (both strands)
     uint32_t best, plus;    // best-stratum mode (bc_align_batch_best): per read only the hits with d <= min(d_min + plus, z)
-    uint32_t ld_policy;     // LD of bc_load_block: cache policy of the index loads
-    uint32_t wide_s;        // LD 2: interval widths from here on are "the top of the trees" (L2 evict-last)
+    uint32_t ld_policy;     // LD of bc_ld256: cache policy of the index loads
 };
 
 // launchers (return cudaError_t of the launch)
