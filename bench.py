@@ -330,15 +330,16 @@ def measure(name: str, args, dev, rank: int, world: int, steps: int, warmup: int
                          "pool_entries_per_warp": stats["geometry"] & 0xFFFF},
             "note": ("algorithmic bytes = 32 B x index blocks the search must read (1 or 2 per node, counted by the kernel) / "
                      "search-kernel time from CUDA events on its stream; peak = measured streaming HBM bandwidth.  ") +
-                    ("The index is far beyond L2: rank queries go to HBM, where every missing 32-byte block costs a whole "
-                     "128-byte line (profiles/r02_random_line_ncu.md), so traffic_over_algorithmic cannot drop below ~2-3 with "
-                     "this block size; see dram_lines." if hbm_regime else
+                    ("The index is far beyond L2: rank queries go to HBM.  With default cache policies every missing 32-byte "
+                     "block costs a whole 128-byte line; the kernel's loads carry the 64-byte L2 prefetch-size hint, which halves "
+                     "that (profiles/r02_random_access_ncu.md).  What binds is the RATE of random DRAM accesses, not their bytes: "
+                     "see dram_accesses and random_access_probe." if hbm_regime else
                      "This workload's index is L2-resident (DRAM traffic ~0): HBM does not bind it, instruction issue and L2 "
                      "latency do; frac is reported against the HBM peak only for comparability.")}
     if tr:
-        lines = tr["dram_bytes"] / 128.0
-        roof["dram_lines"] = {"line_bytes": 128, "lines_per_launch": lines, "lines_per_s": lines / k_s,
-                              "dram_bytes_per_s": tr["dram_bytes"] / k_s, "frac_of_hbm_peak_at_the_pins": tr["dram_bytes"] / k_s / 1e9 / peak}
+        acc = tr["dram_bytes"] / 64.0
+        roof["dram_accesses"] = {"access_bytes": 64, "per_launch": acc, "per_s": acc / k_s,
+                                 "dram_bytes_per_s": tr["dram_bytes"] / k_s, "frac_of_hbm_peak_at_the_pins": tr["dram_bytes"] / k_s / 1e9 / peak}
     rec = {
         "value": count * world * steps / (t_ms * 1e-3), "unit": UNIT, "ms_per_step": t_ms / steps,
         "ms_per_step_best": min(step_ms), "ms_per_step_median": float(np.median(step_ms)),
@@ -452,18 +453,25 @@ def run_ours(args):
     # ---- measured random-access rates (the metric's own denominator), outside the timed region ----
     if not args.no_probe:
         idx_bytes = int(out["config"]["index_bytes"])
-        rs_res = bc.bc_measure_random_sectors(min(idx_bytes, 8 << 30), 512, dev)
-        rs_hbm = bc.bc_measure_random_sectors(8 << 30, 256, dev)
+        rs_res = bc.bc_measure_random_sectors(min(idx_bytes, 8 << 30), 512, dev, ld_policy=1)
+        rs_hbm = bc.bc_measure_random_sectors(8 << 30, 256, dev, ld_policy=1)
+        rs_hbm0 = bc.bc_measure_random_sectors(8 << 30, 256, dev, ld_policy=0)
         sect_s = stats["lines"] / k_s if k_s else 0.0
-        out["random_access_probe"] = {
+        probe = {
             "unit": "G loads/s (one 32-byte block each)", "search_kernel_blocks": sect_s / 1e9,
             "probe_index_sized_table": rs_res / 1e9, "probe_8GiB_table_hbm": rs_hbm / 1e9,
-            "probe_8GiB_dram_bytes_per_s_at_128B_per_load": rs_hbm * 128,
-            "how": "bc_measure_random_sectors: 64 warps/SM, 4 independent 256-bit loads in flight per thread, uniformly random "
-                   "32-byte blocks; ncu shows 3.96 DRAM sectors per such load on the 8 GiB table, i.e. every miss fetches a "
-                   "whole 128-byte line (profiles/r02_random_line_ncu.md).  The search kernel beats the probe's block rate "
-                   "because part of its blocks are L1/L2 hits (top of the search trees) and both ends of a narrow interval "
-                   "share a line."}
+            "probe_8GiB_table_hbm_default_cache_policy": rs_hbm0 / 1e9,
+            "how": "bc_measure_random_sectors2: 64 warps/SM, 4 independent 256-bit loads in flight per thread, uniformly random "
+                   "32-byte blocks, the search kernel's load policy (no L1 allocation, 64-byte L2 prefetch size).  ncu on the "
+                   "8 GiB table: 1.99 DRAM sectors per load with that policy, 3.96 with the default one, the SAME loads/s "
+                   "(profiles/r02_random_access_ncu.md): on B200 random HBM access is bound by the access RATE (~44 G/s), not "
+                   "by bytes.  The kernel's block rate exceeds the probe's because part of its blocks are L1/L2 hits (top of "
+                   "the search trees) and both ends of a narrow interval share an access."}
+        da = out["roofline"].get("dram_accesses")
+        if da:
+            probe["search_kernel_dram_accesses"] = da["per_s"] / 1e9
+            probe["frac_of_random_access_rate"] = da["per_s"] / rs_hbm
+        out["random_access_probe"] = probe
     # ---- optional: K batches streamed end to end, H2D of batch b+1 overlapped with the search of batch b ----
     if args.batches > 1:
         genome, first, count, opts, ws, best = ctx["genome"], ctx["first"], ctx["count"], ctx["opts"], ctx["ws"], ctx["best"]

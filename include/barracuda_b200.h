@@ -219,6 +219,10 @@ int bc_index_build_gpu(const uint8_t *text, uint64_t n, uint32_t occ_interval, u
  * d_sink: DEVICE, >= 4 bytes; sectors_per_second: HOST out.  Not part of the hot path. */
 int bc_measure_random_sectors(const void *d_table, size_t table_bytes, uint32_t loads_per_thread, void *d_sink,
                               void *cuda_stream, double *sectors_per_second);
+/* The same with the cache policy of the load chosen: 0 = default (on B200 every L2 miss then fetches the whole
+ * 128-byte line), 1 = the search kernel's default (no L1 allocation, 64-byte L2 prefetch size: 64 bytes per miss). */
+int bc_measure_random_sectors2(const void *d_table, size_t table_bytes, uint32_t loads_per_thread, int ld_policy,
+                               void *d_sink, void *cuda_stream, double *sectors_per_second);
 
 const char *bc_strerror(int status);
 

@@ -107,11 +107,12 @@ def lib():
         L.bc_index_build_gpu_bytes.argtypes = [u64, u32, u32, C.POINTER(C.c_size_t)]
         L.bc_index_build_gpu.argtypes = [vp, u64, u32, u32, vp, C.c_size_t, vp, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_measure_random_sectors.argtypes = [vp, C.c_size_t, u32, vp, vp, C.POINTER(C.c_double)]
+        L.bc_measure_random_sectors2.argtypes = [vp, C.c_size_t, u32, i32, vp, vp, C.POINTER(C.c_double)]
         L.bc_strerror.argtypes = [i32]
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
                   "bc_align_batch", "bc_locate", "bc_last_stats", "bc_set_geometry", "bc_set_tuning", "bc_set_index_layout", "bc_index_build_host",
-                  "bc_index_host_free", "bc_measure_random_sectors", "bc_align_best_workspace_bytes",
+                  "bc_index_host_free", "bc_measure_random_sectors", "bc_measure_random_sectors2", "bc_align_best_workspace_bytes",
                   "bc_align_batch_best", "bc_pair_workspace_bytes", "bc_pair_batch", "bc_index_build_gpu_bytes", "bc_index_build_gpu"):
             getattr(L, f).restype = i32
         _lib = L
@@ -468,8 +469,9 @@ def bc_locate(ix: DeviceIndex, rows, stream=None):
     return pos
 
 
-def bc_measure_random_sectors(table_bytes: int, loads_per_thread: int = 256, device="cuda:0", stream=None) -> float:
-    """Random 32-byte-sector load rate (sectors/s) over a torch-allocated table of `table_bytes`."""
+def bc_measure_random_sectors(table_bytes: int, loads_per_thread: int = 256, device="cuda:0", stream=None, ld_policy: int = 0) -> float:
+    """Random 32-byte-sector load rate (sectors/s) over a torch-allocated table of `table_bytes`; ld_policy 0 =
+    default cache policies, 1 = the search kernel's (no L1 allocation, 64-byte L2 prefetch size)."""
     torch = _torch()
     dev = torch.device(device)
     with torch.cuda.device(dev):
@@ -477,8 +479,8 @@ def bc_measure_random_sectors(table_bytes: int, loads_per_thread: int = 256, dev
         table.fill_(0x5A5A5A5A)
         sink = torch.zeros(4, dtype=torch.int32, device=dev)
         out = C.c_double(0.0)
-        rc = lib().bc_measure_random_sectors(C.c_void_p(table.data_ptr()), table.numel() * 4, loads_per_thread,
-                                             C.c_void_p(sink.data_ptr()), _stream_ptr(torch, stream), C.byref(out))
+        rc = lib().bc_measure_random_sectors2(C.c_void_p(table.data_ptr()), table.numel() * 4, loads_per_thread, ld_policy,
+                                              C.c_void_p(sink.data_ptr()), _stream_ptr(torch, stream), C.byref(out))
     _check(rc, "bc_measure_random_sectors")
     return float(out.value)
 
