@@ -135,11 +135,13 @@ int bc_align_batch(const bc_index *ix, const bc_reads *reads, const bc_opts *o, 
 /* Best-stratum mode (the early-terminating behaviour of production short-read
  * aligners, "85 % match uniquely"): per read, exactly the hits of bc_align_batch whose
  * d <= min(d_min + stratum_plus, z), d_min = the read's smallest d over both strands; reads without
- * a hit within z stay empty.  Computed by iterative deepening over the budget with bc_align_batch
- * as the inner step, so well-matching reads never pay for the deep budgets.  Same buffers, layout,
- * ordering and status codes as bc_align_batch (n_hits_needed on BC_E_OVERFLOW refers to the pass
- * that failed); bc_last_stats afterwards holds the sums over the passes and [15] = passes run.
- * hits_capacity in the *_bytes call must be the capacity later passed in bc_result. */
+ * a hit within z stay empty.  Computed INSIDE the persistent search kernel: every read is searched with its own
+ * budget 0, 1, 2, ... by the warp that drew it until its first hits appear (they all have d = d_min), then once
+ * more with min(d_min + stratum_plus, z); one launch of the hot path, so well-matching reads never pay for the deep
+ * budgets and nothing waits on the host.  Same buffers, layout, ordering and status codes as bc_align_batch (the
+ * raw-hit arena also holds the first-hit round's records, which the final round repeats);
+ * bc_last_stats[15] = largest per-read budget searched + 1.  bc_align_best_workspace_bytes = bc_align_workspace_bytes
+ * (hits_capacity is ignored; kept for source compatibility). */
 int bc_align_best_workspace_bytes(const bc_index *ix, uint32_t n_reads, uint32_t max_len, const bc_opts *o,
                                   uint32_t raw_hits_per_read, uint64_t hits_capacity, size_t *bytes);
 int bc_align_batch_best(const bc_index *ix, const bc_reads *reads, const bc_opts *o, int32_t stratum_plus,
