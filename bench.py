@@ -348,7 +348,7 @@ def measure(name: str, args, dev, rank: int, world: int, steps: int, warmup: int
                    "index_bytes": index_bytes, "l2": "flushed between steps (256 MiB fill, untimed)",
                    "parallelism": f"dp{world} (index replicated, reads sharded, no collective)",
                    "hits_per_step": n_hits, "index_build": index_build,
-                   "mode": ("best-stratum +%d (bc_align_batch_best, budgets 0..%d in one launch)" % (args.best, max(0, stats.get("passes", 1) - 1))) if best else "exhaustive (bc_align_batch)"},
+                   "mode": ("best-stratum +%d (bc_align_batch_best, budgets 0..%d in one launch)" % (args.best, max(0, stats.get("passes_or_steals", 1) - 1))) if best else "exhaustive (bc_align_batch)"},
         "e2e": {"value": count * world * len(e2e_times) / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": KERNELS_PER_STEP * steps,         # both modes: one launch of the hot path per step
         "clocks": clocks, "roofline": roof,

@@ -114,6 +114,12 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 // Per warp: a RING of BRANCH states (some difference is affordable at their position), whose cold bottom
 // spills to global memory in blocks of 32, and two stacks of RUN states (see the kernel's comment).
 #define BC_FREE_BIT 0x40000000u
+#ifndef BC_POLLERS_PER_CTA
+#define BC_POLLERS_PER_CTA 1u          /* idle warps per CTA that stay to take donated blocks (build-time gene) */
+#endif
+#ifndef BC_POLL_NS
+#define BC_POLL_NS 2000
+#endif
 #ifndef BC_SEARCH_MAX_THREADS
 #define BC_SEARCH_MAX_THREADS 256
 #endif
@@ -527,7 +533,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
             flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill, bc_unit_sectors<LAY>());
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             if (lane == 0) {
-                if (!(warp_flags[warp] & WF_POLLER) && atomicCAS(&cta_poller, 0u, 1u) == 0u) warp_flags[warp] |= WF_POLLER;
+                if (!(warp_flags[warp] & WF_POLLER) && atomicAdd(&cta_poller, 1u) < BC_POLLERS_PER_CTA) warp_flags[warp] |= WF_POLLER;
                 __threadfence();
                 atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);
                 warp_flags[warp] |= WF_COUNTED;
@@ -581,7 +587,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                     }
                     if (lane == 0) atomicAdd(&ctr[BC_CTR_GIDLE], 1ull);
                 } else if (idle >= started) break;
-                __nanosleep(2000);
+                __nanosleep(BC_POLL_NS);
             }
             if (!got) break;
             continue;
