@@ -115,10 +115,10 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 // spills to global memory in blocks of 32, and two stacks of RUN states (see the kernel's comment).
 #define BC_FREE_BIT 0x40000000u
 #ifndef BC_POLLERS_PER_CTA
-#define BC_POLLERS_PER_CTA 1u          /* idle warps per CTA that stay to take donated blocks (build-time gene) */
+#define BC_POLLERS_PER_CTA 8u          /* idle warps per CTA that stay to take donated blocks (build-time gene; measured 1 / 3 / 8) */
 #endif
 #ifndef BC_POLL_NS
-#define BC_POLL_NS 2000
+#define BC_POLL_NS 8000
 #endif
 #ifndef BC_SEARCH_MAX_THREADS
 #define BC_SEARCH_MAX_THREADS 256
@@ -368,7 +368,7 @@ template <bool SMALL, bool HAS_N, int LD, int LAY>
 __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
-    __shared__ uint32_t cta_poller;                                          // this CTA has a warp that takes donated work
+    __shared__ uint32_t cta_poller;                                          // warps of this CTA that have become pollers
     // rarely touched per-lane / per-warp variables live in shared memory, not in registers of the hot loop:
     __shared__ uint2 best_lane[BC_SEARCH_MAX_THREADS];                       // best mode: {read, budget | state << 8} of this lane's read
     __shared__ uint32_t warp_flags[BC_SEARCH_MAX_THREADS / 32];              // bit 0 poller, 1 counted idle, 2 best mode done
@@ -529,7 +529,8 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
         if (bcnt == 0 && c0 + c1 == 0) {
             if (more || (best && !(warp_flags[warp] & WF_BESTDONE))) continue;   // (best mode: the round logic above decides when the warp is done)
             if (!QN) break;
-            // ---- out of work.  Count this warp idle; the first idle warp of the CTA becomes its poller, the others leave.
+            // ---- out of work.  Count this warp idle; up to BC_POLLERS_PER_CTA idle warps of a CTA (default: all) stay as
+            // pollers, further ones leave.
             flush_stats(ctr, lane, n_cnodes, n_xsect, n_bsteps, n_bnodes, n_csteps, n_cancel, n_spill, bc_unit_sectors<LAY>());
             n_cnodes = n_xsect = n_bsteps = n_bnodes = n_csteps = n_cancel = n_spill = 0;
             if (lane == 0) {
@@ -557,7 +558,7 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
                 idle = __shfl_sync(0xffffffffu, idle, 0); ready = __shfl_sync(0xffffffffu, ready, 0);
                 err = __shfl_sync(0xffffffffu, err, 0); started = __shfl_sync(0xffffffffu, started, 0);
                 if (err) break;
-                if (++spins > (1u << 28)) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // ~10 min: a bug, not a wait
+                if (++spins > (1u << 27)) { if (lane == 0) atomicOr(&ctr[BC_CTR_ERROR], 2ull); break; }   // ~18 min of polling: a bug, not a wait
                 if (ready > 0ull) {
                     if (lane == 0) atomicAdd(&ctr[BC_CTR_GIDLE], ~0ull);                  // -1: not idle while claiming
                     uint32_t slot = 0xFFFFFFFFu;
