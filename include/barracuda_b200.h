@@ -214,6 +214,28 @@ int bc_index_build_gpu_bytes(uint64_t n, uint32_t occ_interval, uint32_t sa_inte
 int bc_index_build_gpu(const uint8_t *text, uint64_t n, uint32_t occ_interval, uint32_t sa_interval, void *d_scratch,
                        size_t scratch_bytes, void *cuda_stream, bc_index_host **out);
 
+/* Exclusive scan of n uint32 counts into n+1 uint64 offsets (d_out[0] = 0, d_out[n] = total): the scan of step
+ * A6 (per-query hit counts -> CSR offsets) on its own.  d_in, d_out, d_scratch: DEVICE; d_scratch
+ * 8-byte aligned, >= bc_exclusive_scan_scratch_bytes(n) (BC_E_NOMEM otherwise).  Enqueues three kernels on the
+ * stream and returns without synchronising. */
+size_t bc_exclusive_scan_scratch_bytes(uint64_t n);
+int bc_exclusive_scan_u32(const uint32_t *d_in, uint64_t n, void *d_scratch, size_t scratch_bytes, uint64_t *d_out,
+                          void *cuda_stream);
+
+/* The same scan for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): NO scratch argument -- the per-tile sums live in a static __device__ array inside the library
+ * (262,160 bytes, held by every GPU that loads the library until the process exits), and the call performs no
+ * cudaMalloc / cudaFree / allocating library call.  Limit: n <= bc_scan_static_max_n() = 67,108,864; a larger n
+ * returns BC_E_UNSUPPORTED (use bc_exclusive_scan_u32 with scratch of your own).  The array's device address is
+ * looked up once per device on first use (or by bc_scan_static_setup(), to be called once per device, with that
+ * device current, before a stream capture starts).  All calls on a device SHARE the array and it keeps the last
+ * call's contents; nothing in it needs clearing (every word read is written earlier in the same call), but calls
+ * that overlap on the GPU -- two streams, two threads -- race: serialise them.  Enqueues on the stream and returns
+ * without synchronising; output identical to bc_exclusive_scan_u32's. */
+uint64_t bc_scan_static_max_n(void);
+int bc_scan_static_setup(void);
+int bc_exclusive_scan_u32_static(const uint32_t *d_in, uint64_t n, uint64_t *d_out, void *cuda_stream);
+
 /* Measured denominator of the metric "Occ lookups/s vs the random-sector roofline":
  * every thread issues independent uniformly random 32-byte-aligned 256-bit loads (the access one
  * rank query makes) over d_table; timed with CUDA events on the stream.  d_table: DEVICE, 32-byte

@@ -108,6 +108,15 @@ def lib():
         L.bc_index_build_gpu.argtypes = [vp, u64, u32, u32, vp, C.c_size_t, vp, C.POINTER(C.POINTER(bc_index_host))]
         L.bc_measure_random_sectors.argtypes = [vp, C.c_size_t, u32, vp, vp, C.POINTER(C.c_double)]
         L.bc_measure_random_sectors2.argtypes = [vp, C.c_size_t, u32, i32, vp, vp, C.POINTER(C.c_double)]
+        L.bc_exclusive_scan_scratch_bytes.argtypes = [u64]
+        L.bc_exclusive_scan_scratch_bytes.restype = C.c_size_t
+        L.bc_exclusive_scan_u32.argtypes = [vp, u64, vp, C.c_size_t, vp, vp]
+        L.bc_exclusive_scan_u32_static.argtypes = [vp, u64, vp, vp]
+        L.bc_scan_static_max_n.argtypes = []
+        L.bc_scan_static_max_n.restype = u64
+        L.bc_scan_static_setup.argtypes = []
+        for f in ("bc_exclusive_scan_u32", "bc_exclusive_scan_u32_static", "bc_scan_static_setup"):
+            getattr(L, f).restype = i32
         L.bc_strerror.argtypes = [i32]
         L.bc_strerror.restype = C.c_char_p
         for f in ("bc_index_device_bytes", "bc_index_upload", "bc_index_free", "bc_align_workspace_bytes",
@@ -483,6 +492,44 @@ def bc_measure_random_sectors(table_bytes: int, loads_per_thread: int = 256, dev
                                               C.c_void_p(sink.data_ptr()), _stream_ptr(torch, stream), C.byref(out))
     _check(rc, "bc_measure_random_sectors")
     return float(out.value)
+
+
+def bc_exclusive_scan_u32(counts, scratch=None, stream=None):
+    """Exclusive scan of a uint32 device tensor (int32 view) into n+1 uint64 offsets (int64 view); the scratch is a
+    caller-owned device tensor (allocated here by torch when None).  Enqueues on the stream; no synchronise."""
+    torch = _torch()
+    n = counts.numel()
+    out = torch.empty(n + 1, dtype=torch.int64, device=counts.device)
+    need = int(lib().bc_exclusive_scan_scratch_bytes(n))
+    if scratch is None:
+        scratch = torch.empty(need, dtype=torch.uint8, device=counts.device)
+    with torch.cuda.device(counts.device):
+        rc = lib().bc_exclusive_scan_u32(C.c_void_p(counts.data_ptr() if n else None), n, C.c_void_p(scratch.data_ptr()),
+                                         scratch.numel() * scratch.element_size(), C.c_void_p(out.data_ptr()),
+                                         _stream_ptr(torch, stream))
+    _check(rc, "bc_exclusive_scan_u32")
+    return out
+
+
+def bc_scan_static_max_n() -> int:
+    return int(lib().bc_scan_static_max_n())
+
+
+def bc_exclusive_scan_u32_static(counts, out, stream=None):
+    """The same scan with NO allocation anywhere: scratch in a static device array of the library (n up to
+    bc_scan_static_max_n() = 67,108,864), `out` (int64, n+1) provided by the caller.  Calls that overlap on the GPU
+    race on the shared scratch; calls on one stream are safe."""
+    torch = _torch()
+    n = counts.numel()
+    if out.numel() < n + 1:
+        raise ValueError("out must hold n + 1 offsets")
+    with torch.cuda.device(counts.device):
+        rc = lib().bc_exclusive_scan_u32_static(C.c_void_p(counts.data_ptr() if n else None), n, C.c_void_p(out.data_ptr()),
+                                                _stream_ptr(torch, stream))
+    if rc == BC_E_UNSUPPORTED:
+        raise BcError(rc, f"bc_exclusive_scan_u32_static: n = {n} exceeds the static scratch limit {bc_scan_static_max_n()}")
+    _check(rc, "bc_exclusive_scan_u32_static")
+    return out
 
 
 class BestWorkspace:

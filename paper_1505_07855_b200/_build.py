@@ -9,7 +9,7 @@ import subprocess
 _DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_DIR, "csrc")
 SO = os.path.join(_DIR, "libbarracuda_b200.so")
-SOURCES = ["bc_index.cu", "bc_search.cu", "bc_post.cu", "bc_align.cu", "bc_best.cu", "bc_pair.cu", "bc_build_gpu.cu", "bc_roofline.cu", "bc_index_build.cpp"]
+SOURCES = ["bc_index.cu", "bc_search.cu", "bc_post.cu", "bc_align.cu", "bc_best.cu", "bc_pair.cu", "bc_build_gpu.cu", "bc_roofline.cu", "bc_noalloc.cu", "bc_index_build.cpp"]
 HEADERS = ["bc_internal.cuh", "bc_ws.cuh", "bc_host_index.h", os.path.join("..", "..", "include", "barracuda_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-pthread,-O3", "-shared"]
