@@ -10,7 +10,8 @@ can stand beside the kernel inside one run, and an index (1.5 GB) far beyond the
 metric names ("Occ lookups/s vs HBM random-sector roofline"): 1 Gbp repeat-rich genome, one batch of
 1,000,000 x 100 bp reads of its 8 M, z=5, seed 32/2, 1 gap open, 10 extensions; index built by
 bc_index_build_gpu (untimed).  The same JSON line carries sub-records (`sub`) for config 2 (16 Mbp, index
-L2-resident) and, with --sub 2,5b, config 5b at its full 3.1 Gbp.  N>1: the index is built once on rank 0
+L2-resident) and config 5b at its full 3.1 Gbp (no oracle beside that one unless --sub-oracle: its index alone
+takes 7 minutes of host time; the full-size oracle comparison is profiles/r02_bench_config5b_full.json).  N>1: the index is built once on rank 0
 and broadcast, every rank aligns its own batch of the same recipe (read indices rank*B .. (rank+1)*B), no
 data-path collective (weak scaling).  Prints ONE JSON line on rank 0.
 """
@@ -550,12 +551,17 @@ def run_ours(args):
         sub_args.best = None
         sub_args.batches, sub_args.pair = 1, False
         for name in subs:
-            r2, c2 = measure(name, sub_args, dev, 0, 1, max(3, min(args.steps, 5)), 3, False)
-            small = sd.CONFIGS[name].n <= 200_000_000             # the oracle's index builds in seconds to a minute
-            checks(r2, c2, sub_args, dev, with_oracle=(not args.no_cpu) and (small or args.sub_oracle), sample_target=50_000)
-            out["sub"]["config " + name] = r2
+            c2 = {}
+            try:                                                  # a sub-record must never cost the headline its line
+                r2, c2 = measure(name, sub_args, dev, 0, 1, max(3, min(args.steps, 5)), 3, False)
+                small = sd.CONFIGS[name].n <= 200_000_000         # the oracle's index builds in seconds to a minute
+                checks(r2, c2, sub_args, dev, with_oracle=(not args.no_cpu) and (small or args.sub_oracle), sample_target=50_000)
+                out["sub"]["config " + name] = r2
+            except Exception as e:                                # noqa: BLE001
+                out["sub"]["config " + name] = {"error": f"{type(e).__name__}: {e}"}
             for k in list(c2):
                 c2[k] = None
+            del c2
             torch.cuda.empty_cache()
     print(json.dumps(out), flush=True)
     bdist.finish()
@@ -569,7 +575,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="4", choices=sorted(sd.CONFIGS))
-    ap.add_argument("--sub", default="2", help="comma-separated configs measured as sub-records of the same line (N=1 only)")
+    ap.add_argument("--sub", default="2,5b", help="comma-separated configs measured as sub-records of the same line (N=1 only)")
     ap.add_argument("--sub-oracle", action="store_true", help="run the oracle beside the large sub-records too (3.1 Gbp: ~10 min)")
     ap.add_argument("--reads", type=int, default=None, help="reads per step per GPU (default: the config's batch)")
     ap.add_argument("--genome-bp", type=int, default=None,

@@ -584,8 +584,11 @@ def bc_align_batch_best(ix: DeviceIndex, reads: DeviceReads, opts, stratum_plus:
             continue
         if rc != BC_E_OVERFLOW:
             raise BcError(rc, "bc_align_batch_best")
-        per_read = max(2 * ws.raw_hits_per_read, -(-int(need[1]) // max(1, reads.n_reads)) + 1)
-        cap = max(2 * ws.hits_capacity, int(need[0]) + 1)
+        # need = {hits after dedup (0 when the raw arena overflowed: nothing was sorted), raw hits}: grow what was short
+        per_read = max(ws.raw_hits_per_read, -(-int(need[1]) // max(1, reads.n_reads)) + 1)
+        if per_read == ws.raw_hits_per_read and int(need[0]) <= ws.hits_capacity:
+            per_read *= 2
+        cap = max(ws.hits_capacity, int(need[0]) + 1) if int(need[0]) > ws.hits_capacity else ws.hits_capacity
         ws = BestWorkspace(ix, reads.n_reads, max(1, reads.max_len), opts, per_read, cap)
     raise BcError(BC_E_OVERFLOW, "bc_align_batch_best (after growing)")
 

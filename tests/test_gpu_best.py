@@ -35,7 +35,8 @@ def run_best(ix, codes, opts, plus):
     return o, h, bc.bc_last_stats(ix)
 
 
-@pytest.mark.parametrize("name,n,n_reads", [("2", 2_000_000, 3000), ("3", 3_000_000, 3000), ("1", 1_000_000, 5000)])
+@pytest.mark.parametrize("name,n,n_reads", [("2", 2_000_000, 3000), ("3", 3_000_000, 3000), ("1", 1_000_000, 5000),
+                                             ("5a", 1_000_000, 400)])   # few heavy reads: last-round states change warps
 @pytest.mark.parametrize("plus", [0, 1])
 def test_best_stratum_equals_filtered_exhaustive(name, n, n_reads, plus):
     cfg, p = pair_for(name, n)
@@ -83,6 +84,29 @@ def test_best_stratum_edge_cases():
     d = bc.HostReads(b2, nm, off, ln).to_device()
     ws = bc.BestWorkspace(p.ix, 2000, 51, opts, hits_capacity=100)
     assert bc.bc_align_batch_best_raw(p.ix, d, opts, 1, ws) == bc.BC_E_OVERFLOW
+
+
+def test_best_stratum_with_a_deep_budget():
+    """z >= 9 (the round-1 workspace sizing broke there) and z > 7 (thresholds read from memory, not
+    registers): a small batch, plus 0 / 1 / 2, against the filtered oracle result."""
+    cfg = sd.CONFIGS["1"].scaled(n=5_000)
+    from tests.test_gpu_parity import Pair
+    T = sd.make_genome(cfg)
+    p = Pair(T)
+    rng = np.random.default_rng(21)
+    codes = np.stack([T[int(s0):int(s0) + 26] for s0 in rng.integers(0, T.size - 26, size=64)]).astype(np.uint8)
+    for r in codes[:48]:                                # 0..6 substitutions: d_min varies from read to read
+        for _ in range(int(rng.integers(0, 7))):
+            q = int(rng.integers(0, 26))
+            r[q] = (r[q] + 1 + int(rng.integers(0, 3))) & 3
+    opts = (9, 1, 1, 0, 0, 5)
+    off_o, hits_o = p.oracle.align(codes, opts)
+    for plus in (0, 1, 2):
+        want_off, want_hits = best_filter(off_o, hits_o, opts[0], plus)
+        off_g, hits_g, st = run_best(p.ix, codes, opts, plus)
+        assert np.array_equal(off_g, want_off), plus
+        assert hits_g.tobytes() == want_hits.tobytes(), plus
+    assert len(set(np.diff(off_o.astype(np.int64)).tolist())) > 1
 
 
 def test_best_stratum_and_pairing_with_ragged_lengths_and_N():
