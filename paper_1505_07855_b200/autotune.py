@@ -24,9 +24,9 @@ import paper_1505_07855_b200 as bc
 from . import _build
 
 GENES = {                                   # value 0 = "library default" for the run-time genes
-    "min_ctas": (3, 2, 4),                  # BUILD-time: __launch_bounds__(256, min_ctas)
+    "min_ctas": (4, 3, 5),                  # BUILD-time: __launch_bounds__(224, min_ctas) of the default flavour
     "ctas": (0, 2, 3, 4, 5, 6),             # CTAs per SM launched
-    "warps": (0, 4, 6, 8),                  # warps per CTA
+    "warps": (0, 4, 6, 7, 8),               # warps per CTA (8: the 256-thread flavour, 3 CTAs per SM)
     "pool_kb": (0, 128, 144, 160, 176, 192, 208),   # shared memory per SM given to the state pools
     "ld_policy": (0, 1, 2),                 # cache policy of the index loads (bc_set_tuning)
     "layout": (0, 1, 2),                    # device index layout (bc_set_index_layout; needs a re-upload)

@@ -57,14 +57,14 @@ struct Geometry { uint32_t ctas, warps, bcap, ccap, spill_blocks; };
 // geometry of the persistent kernel: CTAs per SM, warps per CTA, per-warp branch ring (power of two)
 // and run-stack sizes that fill the shared memory given to the pools
 int choose_geometry(const bc_index *ix, Geometry &g) {
-    g.warps = ix->warps_per_cta ? ix->warps_per_cta : 8;
-    g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 3;
+    g.warps = ix->warps_per_cta ? ix->warps_per_cta : 7;      // 4 CTAs x 7 warps: see the launch bounds in bc_search.cu
+    g.ctas = ix->ctas_per_sm ? ix->ctas_per_sm : 4;
     g.spill_blocks = ix->spill_blocks ? ix->spill_blocks : BC_SPILL_BLOCKS;
     for (;; --g.ctas) {
-        // pool bytes per SM; what is left of the 228 KB stays L1 (query records).  The autotuner's tables
-        // (profiles/r02_autotune_config2.json, _config4.json): 16 MB index 160/176/192 KB -> 92.6/90.3/89.3 ms;
-        // 1.5 GB index 160/176 KB -> 254.4/252.2 ms (L2 misses make L1 count for more there)
-        const size_t total_kb = ix->pool_kb ? ix->pool_kb : (ix->bytes > ((size_t)64 << 20) ? 176 : 192);
+        // pool bytes per SM; what is left of the shared memory / L1 array stays L1 (query records).  The autotuner's
+        // tables with 4 x 7 warps (profiles/r02_autotune_config2.json, _config4.json): 16 MB index 192 / 208 KB ->
+        // 85.1 / 83.4 ms; 1.5 GB index 160 / 176 / 208 KB -> 254.3 / 248.8 / 256.3 ms (L2 misses make L1 count there)
+        const size_t total_kb = ix->pool_kb ? ix->pool_kb : (ix->bytes > ((size_t)64 << 20) ? 176 : 208);
         size_t budget = total_kb * 1024 / g.ctas;
         if (budget > 200 * 1024) budget = 200 * 1024;
         uint32_t per_warp = (uint32_t)(budget / ((size_t)g.warps * BC_POOL_ENTRY_BYTES));

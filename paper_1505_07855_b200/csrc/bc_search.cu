@@ -120,11 +120,15 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 #ifndef BC_POLL_NS
 #define BC_POLL_NS 8000
 #endif
+// Launch bounds (build-time genes of the autotuner).  The default flavour is compiled for up to 7 warps per CTA and
+// 4 CTAs per SM (28 warps per SM at 72 registers: measured -2.8 % time on config 2 and -2.0 % on config 4 against 3 x 8
+// warps at 80 registers; 5 x 6 and 6 x 5 warps at 64 registers spill and lose 6-7 %); a second flavour (256 threads,
+// 3 CTAs, 80 registers) serves geometries with 8 warps per CTA.
 #ifndef BC_SEARCH_MAX_THREADS
-#define BC_SEARCH_MAX_THREADS 256
+#define BC_SEARCH_MAX_THREADS 224
 #endif
 #ifndef BC_SEARCH_MIN_CTAS
-#define BC_SEARCH_MIN_CTAS 3
+#define BC_SEARCH_MIN_CTAS 4
 #endif
 
 __device__ __forceinline__ void ent_store(uint2 *P, uint32_t idx, uint32_t qid, uint32_t k, uint32_t s, uint32_t k2,
@@ -364,14 +368,14 @@ __device__ __forceinline__ void push_roots(const BcSearchParams &p, bool want, u
 // free and comes back when the ring runs low; if that area is ever full the warp raises error bit 2
 // (BC_E_NOMEM: the caller passes a larger spill area), never a silent truncation.
 // ---------------------------------------------------------------------------------------------
-template <bool SMALL, bool HAS_N, int LD, int LAY>
-__global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
+template <bool SMALL, bool HAS_N, int LD, int LAY, bool W8>
+__global__ void __launch_bounds__(W8 ? 256 : BC_SEARCH_MAX_THREADS, W8 ? 3 : BC_SEARCH_MIN_CTAS) bc_search_kernel(BcSearchParams p) {
     extern __shared__ uint2 pool_mem[];
     __shared__ __align__(16) uint32_t Ctab[8];                               // C[c] of the index each strand searches
     __shared__ uint32_t cta_poller;                                          // warps of this CTA that have become pollers
     // rarely touched per-lane / per-warp variables live in shared memory, not in registers of the hot loop:
-    __shared__ uint2 best_lane[BC_SEARCH_MAX_THREADS];                       // best mode: {read, budget | state << 8} of this lane's read
-    __shared__ uint32_t warp_flags[BC_SEARCH_MAX_THREADS / 32];              // bit 0 poller, 1 counted idle, 2 best mode done
+    __shared__ uint2 best_lane[256];                       // best mode: {read, budget | state << 8} of this lane's read
+    __shared__ uint32_t warp_flags[8];              // bit 0 poller, 1 counted idle, 2 best mode done
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t BCAP = p.bcap, CCAP = p.ccap, BM = p.bcap - 1u;
     uint2 *P = pool_mem + (size_t)warp * 3u * (BCAP + CCAP);     // branch ring: slots (bb + i) & BM
@@ -792,12 +796,18 @@ __global__ void __launch_bounds__(BC_SEARCH_MAX_THREADS, BC_SEARCH_MIN_CTAS) bc_
 #undef WF_BESTDONE
 }
 
+template <bool SMALL, bool HAS_N, int LD, int LAY, bool W8>
+cudaError_t launch_search_w(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
+    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N, LD, LAY, W8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    bc_search_kernel<SMALL, HAS_N, LD, LAY, W8><<<grid, threads, smem, st>>>(p);
+    return cudaGetLastError();
+}
+
 template <bool SMALL, bool HAS_N, int LD, int LAY>
 cudaError_t launch_search(const BcSearchParams &p, int grid, int threads, size_t smem, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(bc_search_kernel<SMALL, HAS_N, LD, LAY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    bc_search_kernel<SMALL, HAS_N, LD, LAY><<<grid, threads, smem, st>>>(p);
-    return cudaGetLastError();
+    if (threads > BC_SEARCH_MAX_THREADS) return launch_search_w<SMALL, HAS_N, LD, LAY, true>(p, grid, threads, smem, st);
+    return launch_search_w<SMALL, HAS_N, LD, LAY, false>(p, grid, threads, smem, st);
 }
 
 template <bool SMALL, bool HAS_N>
