@@ -180,13 +180,14 @@ int bc_locate(const bc_index *ix, const uint32_t *d_rows, uint64_t n_rows, uint3
  * from a busy warp to an idle one; bc_align_batch_best: largest per-read budget searched + 1. */
 int bc_last_stats(const bc_index *ix, uint64_t *out16);
 
-/* Tuning knobs of the persistent search kernel (0 = default): CTAs per SM (<= 8), warps per CTA (<= 8). */
+/* Tuning knobs of the persistent search kernel (0 = default: 4 CTAs per SM of 7 warps): CTAs per SM (<= 8),
+ * warps per CTA (<= 8; 8 selects the kernel flavour compiled for 256 threads and 3 resident CTAs per SM). */
 int bc_set_geometry(bc_index *ix, uint32_t ctas_per_sm, uint32_t warps_per_cta);
 
 /* More tuning (0 = default): spill_blocks = per-warp spill area of the branch rings in blocks of 32
  * states (default 128; bc_align_batch returns BC_E_NOMEM when a warp's area runs full -- raise it, ask
  * bc_align_workspace_bytes again and repeat the call); pool_kb = shared memory per SM given to the
- * state pools, 16..220 KB (default: 192 KB for an L2-resident index, 160 KB beyond); ld_policy = cache
+ * state pools, 16..220 KB (default: 208 KB for an index up to 64 MB, 176 KB beyond); ld_policy = cache
  * policy of the index loads: 1 = default policies, 2 = no L1 allocation + 64-byte L2 prefetch size (the library
  * default); ld_policy + 256 switches the exchange of pending states between warps off (A/B measurements).
  * spill_blocks affects the workspace size: set it before bc_align_workspace_bytes. */
