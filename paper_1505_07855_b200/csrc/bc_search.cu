@@ -398,9 +398,10 @@ __global__ void __launch_bounds__(W8 ? 256 : BC_SEARCH_MAX_THREADS, W8 ? 3 : BC_
     if (threadIdx.x < 8) Ctab[threadIdx.x] = p.ix.bwt[threadIdx.x < 4 ? 1 : 0].C[threadIdx.x & 3];
     if (threadIdx.x == 0) cta_poller = 0u;
     __syncthreads();
-    // A4, state-level redistribution ACROSS warps (exhaustive mode): a busy warp that is about to spill the bottom of
-    // its ring gives that block of 32 pending states away instead, if some warp has run out of work; the first
-    // idle warp of every CTA stays behind as its CTA's "poller" and takes such blocks.  See steal_* below.
+    // A4, state-level redistribution ACROSS warps: a busy warp that is about to spill the bottom of its ring gives that
+    // block of 32 pending states away instead (through the exchange buffer of the workspace) if some warp has run out
+    // of work; warps that are out of work stay behind as pollers and take such blocks (protocol and termination: the
+    // "out of work" branch of the main loop, and DESIGN.md 6).  Only blocks whose 32 states all carry BC_FREE_BIT move.
 #define QN (p.ws.sq_n)                                /* read from the parameter bank where needed: no register */
 #define sq_flag ((volatile uint32_t *)p.ws.sq_flag)  /* per slot: 0 free, 3 being written, 1 ready, 2 being read */
     best_lane[threadIdx.x] = make_uint2(0u, 0u);     // state 0 free / 1 searching for the first hit / 2 final round
