@@ -34,6 +34,7 @@ int make_ws_layout(uint32_t n_reads, uint32_t max_len, const bc_opts *o, bool wi
     L.spill_blocks = spill_blocks;
     qrec_layout(o, max_len, true, L);
     const size_t qrec_bytes = (size_t)L.nq * L.qstride;
+    if (qrec_bytes >= ((size_t)1 << 34)) return BC_E_INVAL;      // the kernel indexes record words with 32 bits
     qrec_layout(o, max_len, with_n, L);
     size_t x = 0;
     L.off_qrec = x;    x = align_up(x + qrec_bytes, 256);

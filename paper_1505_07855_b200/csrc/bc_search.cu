@@ -117,6 +117,9 @@ __device__ __forceinline__ uint32_t sel4(uint32_t a0, uint32_t a1, uint32_t a2, 
 #ifndef BC_POLLERS_PER_CTA
 #define BC_POLLERS_PER_CTA 8u          /* idle warps per CTA that stay to take donated blocks (build-time gene; measured 1 / 3 / 8) */
 #endif
+#ifndef BC_FAIR_DIV
+#define BC_FAIR_DIV 4                   /* intake draws at most (queries left) / (BC_FAIR_DIV x warps) + 1 at a time (build-time gene) */
+#endif
 #ifndef BC_POLL_NS
 #define BC_POLL_NS 8000
 #endif
@@ -205,6 +208,20 @@ __device__ __forceinline__ uint32_t q_base(const uint8_t *rec, uint32_t boff, ui
     }
     return c;
 }
+// the same by query number, with 32-bit word arithmetic (the host refuses batches whose records exceed 2^34 bytes)
+template <bool HAS_N>
+__device__ __forceinline__ uint32_t q_base_at(const uint8_t *qrec, uint32_t qid, uint32_t qstride, uint32_t boff, uint32_t noff,
+                                              uint32_t t) {
+    const uint32_t *W = reinterpret_cast<const uint32_t *>(qrec);
+    const uint32_t r = qid * (qstride >> 2);
+    const uint32_t w = __ldg(W + (r + (boff >> 2) + (t >> 4)));
+    uint32_t c = (w >> (2u * (t & 15u))) & 3u;
+    if (HAS_N) {
+        const uint32_t nm = __ldg(W + (r + (noff >> 2) + (t >> 5)));
+        if ((nm >> (t & 31u)) & 1u) c = 4u;
+    }
+    return c;
+}
 
 // First position at which a state with `rem` differences left, seed differences sdc can afford ANY difference:
 // before it the D / Ds bounds (or a spent seed budget) leave exact matching as the only move.  rem == 0: the
@@ -287,13 +304,13 @@ __device__ __forceinline__ void chain_steps(const BcSearchParams &p, const uint4
                     const uint32_t dollar = s - (phi - plo), nx = xhi - xlo, nc_ = ohi - olo;
                     k2 = c == 0u ? k2 + dollar : (c == 1u ? k2 + dollar + nx : (c == 2u ? k2 + s - nx - nc_ : k2 + s - nc_));
                 }
-                k = Cs[c] + olo + 1u; s = ohi - olo; ++t;
+                k = p.ix.bwt[S0 ? 1 : 0].C[c] + olo + 1u; s = ohi - olo; ++t;
                 const bool done = t == te;
                 emit = done && t == m; toring = done && !emit; alive = !done;
             }
         }
         uint32_t nb = 0;
-        if (alive) nb = q_base<HAS_N>(p.ws.qrec + (size_t)qid * p.ws.qstride, p.ws.q_boff, p.ws.q_noff, t);
+        if (alive) nb = q_base_at<HAS_N>(p.ws.qrec, qid, p.ws.qstride, p.ws.q_boff, p.ws.q_noff, t);
         const uint32_t smask = __ballot_sync(0xffffffffu, alive);
         if (alive) {
             const uint32_t r = __popc(smask & lt_mask);
@@ -472,7 +489,7 @@ __global__ void __launch_bounds__(W8 ? 256 : BC_SEARCH_MAX_THREADS, W8 ? 3 : BC_
                     // trees are spread over the warps instead of queueing behind one another
                     const unsigned long long seen = *(volatile unsigned long long *)&ctr[BC_CTR_TICKET];
                     const unsigned long long left = seen < nq ? nq - seen : 0ull;
-                    const unsigned long long fair = left / (4ull * gridDim.x * (blockDim.x >> 5)) + 1ull;
+                    const unsigned long long fair = left / ((unsigned long long)BC_FAIR_DIV * gridDim.x * (blockDim.x >> 5)) + 1ull;
                     if (fair < need) need = (uint32_t)fair;
                     tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);
                 }
@@ -509,7 +526,7 @@ __global__ void __launch_bounds__(W8 ? 256 : BC_SEARCH_MAX_THREADS, W8 ? 3 : BC_
                 if (lane == 0) {
                     const unsigned long long seen = *(volatile unsigned long long *)&ctr[BC_CTR_TICKET];
                     const unsigned long long left = seen < n_reads ? n_reads - seen : 0ull;
-                    const unsigned long long fair = left / (4ull * gridDim.x * (blockDim.x >> 5)) + 1ull;
+                    const unsigned long long fair = left / ((unsigned long long)BC_FAIR_DIV * gridDim.x * (blockDim.x >> 5)) + 1ull;
                     if (fair < need) need = (uint32_t)fair;
                     tk = atomicAdd(&ctr[BC_CTR_TICKET], (unsigned long long)need);     // tickets are READS in this mode
                 }
